@@ -1,0 +1,160 @@
+/*
+ * photons.h — C ABI of the B200-native truncated short-range gravity P2P library.
+ *
+ * What the library computes (§2, Eq. 1; BASELINE.json north_star):
+ *
+ *   a_i = G * sum_{j != i, 0 < |d_ij| < r_cut}  m_j * d_ij * g(|d_ij|) / |d_ij|^3
+ *   g(r) = erfc(r / 2 r_s) + r / (r_s sqrt(pi)) * exp(-r^2 / 4 r_s^2)              (Eq. 1)
+ *   r_s  = rs_over_cell * boxsize / n_pm   (1.2 cells, L33),  r_cut = rcut_over_rs * r_s (6, L53/L143)
+ *   d_ij = minimum image of (r_j - r_i) in the periodic cube of side boxsize
+ *
+ * evaluated the paper's way (§3, Alg. 1/2): particles sorted into the leaves of an ORB tree
+ * (<= maxleaf particles each, L35), every target leaf summing over the source leaves whose
+ * periodic bounding boxes come within r_cut of its own (the "P2P task list", L65, L77-L85).
+ *
+ * Conventions for every entry point
+ *   - plain C: no C++ types, no exceptions cross this boundary; every call returns a PHOTONS_* status;
+ *     out-parameters are untouched on error; photons_last_error() gives the message.
+ *   - "host or device" pointers are tagged by a PHOTONS_MEM_* argument.  The caller owns pos, mass and
+ *     acc; the library copies inputs inside photons_set_particles and keeps no caller pointer.
+ *   - the context owns all device buffers and CUDA streams; a context is not thread-safe; different
+ *     contexts are independent.
+ *   - call order: create -> set_particles -> build_leaves -> short_range_acc (repeatable);
+ *     set_particles invalidates the leaves.  A call out of order returns PHOTONS_ESTATE.
+ *   - there is no CPU fallback: without a CUDA device photons_create fails with PHOTONS_ENODEVICE.
+ */
+#ifndef PHOTONS_H
+#define PHOTONS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct photons_ctx photons_ctx; /* opaque; owned by the library */
+
+enum {
+    PHOTONS_OK = 0,
+    PHOTONS_EINVAL = 1,     /* bad argument or parameter */
+    PHOTONS_ESTATE = 2,     /* call out of order */
+    PHOTONS_ENOMEM = 3,     /* host or device allocation failed */
+    PHOTONS_ECUDA = 4,      /* CUDA runtime error (message in photons_last_error) */
+    PHOTONS_ENODEVICE = 5,  /* no usable CUDA device */
+    PHOTONS_EBOX = 6,       /* r_cut >= boxsize/2, or 2 r_cut + leaf extents >= boxsize (minimum image
+                               per list entry would be ambiguous; A10) */
+    PHOTONS_ENONFINITE = 7  /* NaN/Inf in positions or masses */
+};
+
+/* precision of the P2P path (SP and DP runs; "mixed": north_star) */
+enum {
+    PHOTONS_FP64 = 0,   /* fp64 positions, fp64 pair arithmetic */
+    PHOTONS_FP32 = 1,   /* absolute positions stored in fp32, fp32 pair arithmetic */
+    PHOTONS_MIXED = 2   /* fp32 offsets from the leaf centre (centres and centre differences in fp64),
+                           fp32 pair arithmetic */
+};
+
+/* how the truncation function g is evaluated inside the pair core (§3.3) */
+enum {
+    PHOTONS_G_DIRECT = 0, /* erfc/exp special functions per pair (what §3.3 L121 calls expensive) */
+    PHOTONS_G_TABLE = 1,  /* Eq. 2 (L127-L143): table {T_i, E_i} in shared memory + Taylor terms T[0..level] */
+    PHOTONS_G_POLY = 2    /* no table, no special function: g/r^3 = 1/r^3 - Q(s)/(2 r_s)^3 with
+                             s = (r/2r_s)^2 and Q an FMA-pipe polynomial (fp32 paths only) */
+};
+
+enum { PHOTONS_MEM_HOST = 0, PHOTONS_MEM_DEVICE = 1 };
+
+/* element type of caller arrays (pos, mass, acc) */
+enum { PHOTONS_DTYPE_F64 = 0, PHOTONS_DTYPE_F32 = 1 };
+
+typedef struct {
+    double boxsize;           /* > 0; period of the cube */
+    int n_pm;                 /* PM mesh cells per side (L33); must give r_cut < boxsize/2 */
+    double rs_over_cell;      /* split radius in cells: 1.2 (L33) */
+    double rcut_over_rs;      /* cut-off in r_s: 6.0 (north_star; the table spans x = r/2r_s in [0,3], L143);
+                                 must be <= 6 for g_mode TABLE and POLY (their range), any value for DIRECT */
+    double G;                 /* gravitational constant */
+    int maxleaf;              /* MAXLEAF (L35): 16, 32, 64 or 128 */
+    int precision;            /* PHOTONS_FP64 / FP32 / MIXED */
+    int g_mode;               /* PHOTONS_G_* */
+    int table_nodes;          /* TABLE: number of intervals n over x in [0,3] (n+1 nodes), 64..4096; paper: 512 */
+    int table_level;          /* TABLE: highest Taylor term kept, 0..4 (paper: T[2] for SP, T[4] for DP, L149) */
+    int n_streams;            /* >= 1: target-leaf batches are issued round-robin over this many CUDA streams */
+    int device;               /* CUDA device ordinal */
+    double close_pair_radius; /* fp32/mixed paths: pairs with 0 < r < this are evaluated in fp64 inside the
+                                 kernel (A12); 0 = off.  Ignored by PHOTONS_FP64. */
+    int chunk_max;            /* largest number of source particle slots staged per shared-memory stage;
+                                 0 = default (128); multiple of maxleaf, <= 256 */
+    int warps_per_leaf;       /* warps of the CTA that owns one target leaf; they split its source list.
+                                 0 = default; 1, 2, 4 or 8 */
+    int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (13) */
+} photons_params;
+
+typedef struct {
+    long long n_particles;
+    long long n_leaves;        /* leaves of the ORB tree (all at the same depth) */
+    long long n_chunks;        /* interaction-list entries: runs of contiguous source leaves, <= chunk_max slots */
+    long long n_leaf_pairs;    /* (target leaf, source leaf) tasks, the paper's Task list length (L77) */
+    long long pairs_evaluated; /* sum over tasks of n_i * n_j, real particles only (paper's count, L218; A18) */
+    long long max_leaves_per_target; /* longest source list, in leaves */
+    double build_ms;           /* last photons_build_leaves, host wall clock incl. device sync */
+    double kernel_ms;          /* last photons_short_range_acc: CUDA-event time of the P2P launches alone */
+    double total_ms;           /* last photons_short_range_acc: host wall clock incl. copies and sync */
+} photons_stats;
+
+/* Fill *p with the paper's defaults: boxsize 1, n_pm 32, rs_over_cell 1.2, rcut_over_rs 6, G 1, maxleaf 32,
+ * FP32, G_POLY, table 512/level 2, 1 stream, device 0, close pairs off, chunk_max default. */
+void photons_default_params(photons_params* p);
+
+/* Validate parameters, select the device, create streams, build the g table (TABLE mode; fp64 on the
+ * host, rounded once).  Errors: EINVAL, EBOX (r_cut >= boxsize/2), ENODEVICE, ECUDA, ENOMEM.
+ * On error *out is untouched and, if err_buf != NULL, a message is written there (err_len bytes). */
+int photons_create(const photons_params* p, photons_ctx** out, char* err_buf, int err_len);
+
+/* Copy n particles in.  pos: n x 3 row-major, mass: n values or NULL (= 1/n each), both of element type
+ * dtype (PHOTONS_DTYPE_*), both host or both device memory as tagged.  Positions are wrapped into
+ * [0, boxsize).  cuda_stream: a cudaStream_t the device-side copy is ordered after (NULL = default stream);
+ * the call returns after the copy has completed.  Errors: EINVAL (n < 1, or more than 2^31 - 1 particle slots),
+ * ENONFINITE, ENOMEM, ECUDA. */
+int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const void* mass, int dtype,
+                          int mem_kind, void* cuda_stream);
+
+/* ORB sort (L35) -> leaf-sorted packed particle arrays in the path's precision (SoA by leaf, L69),
+ * leaf table (L79: first slot, count; plus tight bounding boxes), interaction list grouped by target leaf
+ * with the periodic image shift of every entry (the paper's TaskGroup/GroupIdx, L83-L85).  All on the
+ * device.  Errors: ESTATE, EBOX, ENOMEM, ECUDA. */
+int photons_build_leaves(photons_ctx* ctx);
+
+/* The P2P kernel (Alg. 1 + Alg. 2): acc[n x 3] row-major in the CALLER's particle order, element type
+ * dtype, host or device memory.  stats may be NULL.  Errors: ESTATE, EINVAL, ECUDA. */
+int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind, photons_stats* stats);
+
+/* Test hooks (host output buffers).  perm[q] = caller index of the particle at leaf-sorted position q
+ * (n entries); leaf_start[k] = first sorted position of leaf k (n_leaves + 1 entries).  Either may be NULL. */
+int photons_get_leaf_order(photons_ctx* ctx, long long* perm, long long* leaf_start);
+
+/* Interaction list as built: chunk_ptr[n_leaves + 1], then per chunk: first source leaf, number of source
+ * leaves, shift code (sx+1) + 3*(sy+1) + 9*(sz+1) with s in {-1,0,+1} box lengths added to the source.
+ * Pass NULL pointers to query sizes through stats only. */
+int photons_get_interaction_list(photons_ctx* ctx, long long* chunk_ptr, int* first_leaf, int* n_leaf,
+                                 int* shift_code);
+
+/* Statistics of the last build / run. */
+int photons_get_stats(photons_ctx* ctx, photons_stats* stats);
+
+/* Device throughput micro-benchmarks that give the roofline denominators:
+ * kind 0 = FFMA (register operands), 1 = FFMA2 (fma.rn.f32x2), 2 = DFMA, 3 = MUFU.RSQ,
+ * 4 = FFMA2 with 2 MUFU.RSQ per 8 (FFMA2 lanes counted), 5 = LDS.128 broadcast, 6 = FFMA with immediates,
+ * 7 = FFMA2 with 4 ALU-pipe ops per 8 (FFMA2 lanes counted), 8 = FADD2, 9 = FMUL2, 10 = FFMA2 without
+ * operand reuse.  *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction
+ * counts 2 per lane; multiply FMA rates by 2 for flops).  Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
+int photons_peak_probe(int device, int kind, double* out);
+
+/* Message of the last failing call on ctx; valid until the next call on ctx. */
+const char* photons_last_error(const photons_ctx* ctx);
+
+/* Free everything.  NULL-safe. */
+void photons_destroy(photons_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PHOTONS_H */

@@ -1,0 +1,250 @@
+"""ctypes binding of libphotons.so — argument marshalling only; every step of the path runs in the CUDA
+library (include/photons.h).  PyTorch appears here only as the owner of device memory and streams: tensors
+are passed by ``data_ptr()`` and ``torch.cuda.current_stream().cuda_stream``.
+
+There is no fallback: if the shared library is missing, or there is no CUDA device, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libphotons.so")
+
+OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENODEVICE, EBOX, ENONFINITE = range(8)
+FP64, FP32, MIXED = 0, 1, 2
+G_DIRECT, G_TABLE, G_POLY = 0, 1, 2
+MEM_HOST, MEM_DEVICE = 0, 1
+DTYPE_F64, DTYPE_F32 = 0, 1
+
+PRECISIONS = {"fp64": FP64, "fp32": FP32, "mixed": MIXED}
+G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY}
+ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX", "ENONFINITE"]
+
+EXPORTS = [
+    "photons_default_params", "photons_create", "photons_set_particles", "photons_build_leaves",
+    "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
+    "photons_peak_probe", "photons_last_error", "photons_destroy",
+]
+
+
+class Params(ctypes.Structure):
+    _fields_ = [
+        ("boxsize", ctypes.c_double), ("n_pm", ctypes.c_int), ("rs_over_cell", ctypes.c_double),
+        ("rcut_over_rs", ctypes.c_double), ("G", ctypes.c_double), ("maxleaf", ctypes.c_int),
+        ("precision", ctypes.c_int), ("g_mode", ctypes.c_int), ("table_nodes", ctypes.c_int),
+        ("table_level", ctypes.c_int), ("n_streams", ctypes.c_int), ("device", ctypes.c_int),
+        ("close_pair_radius", ctypes.c_double), ("chunk_max", ctypes.c_int), ("warps_per_leaf", ctypes.c_int),
+        ("poly_degree", ctypes.c_int),
+    ]
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [
+        ("n_particles", ctypes.c_longlong), ("n_leaves", ctypes.c_longlong), ("n_chunks", ctypes.c_longlong),
+        ("n_leaf_pairs", ctypes.c_longlong), ("pairs_evaluated", ctypes.c_longlong),
+        ("max_leaves_per_target", ctypes.c_longlong), ("build_ms", ctypes.c_double),
+        ("kernel_ms", ctypes.c_double), ("total_ms", ctypes.c_double),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class PhotonsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"photons: {ERROR_NAMES[code] if 0 <= code < len(ERROR_NAMES) else code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Load libphotons.so (built by ``python -m paper_2107_14008_b200.build``); raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2107_14008_b200.build` "
+                          "(there is no CPU fallback for the CUDA path)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ll, ci = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int
+    lib.photons_default_params.restype = None
+    lib.photons_default_params.argtypes = [ctypes.POINTER(Params)]
+    lib.photons_create.restype = ci
+    lib.photons_create.argtypes = [ctypes.POINTER(Params), ctypes.POINTER(vp), ctypes.c_char_p, ci]
+    lib.photons_set_particles.restype = ci
+    lib.photons_set_particles.argtypes = [vp, ll, vp, vp, ci, ci, vp]
+    lib.photons_build_leaves.restype = ci
+    lib.photons_build_leaves.argtypes = [vp]
+    lib.photons_short_range_acc.restype = ci
+    lib.photons_short_range_acc.argtypes = [vp, vp, ci, ci, ctypes.POINTER(Stats)]
+    lib.photons_get_leaf_order.restype = ci
+    lib.photons_get_leaf_order.argtypes = [vp, vp, vp]
+    lib.photons_get_interaction_list.restype = ci
+    lib.photons_get_interaction_list.argtypes = [vp, vp, vp, vp, vp]
+    lib.photons_get_stats.restype = ci
+    lib.photons_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
+    lib.photons_peak_probe.restype = ci
+    lib.photons_peak_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.photons_last_error.restype = ctypes.c_char_p
+    lib.photons_last_error.argtypes = [vp]
+    lib.photons_destroy.restype = None
+    lib.photons_destroy.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def default_params(**overrides) -> Params:
+    p = Params()
+    load().photons_default_params(ctypes.byref(p))
+    for k, v in overrides.items():
+        if k == "precision" and isinstance(v, str):
+            v = PRECISIONS[v]
+        if k == "g_mode" and isinstance(v, str):
+            v = G_MODES[v]
+        if not hasattr(p, k):
+            raise TypeError(f"unknown parameter {k!r}")
+        setattr(p, k, v)
+    return p
+
+
+def _is_tensor(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _marshal(x, name):
+    """(pointer, dtype code, mem kind, keep-alive object) of a numpy array or a torch tensor."""
+    if _is_tensor(x):
+        import torch
+        if x.dtype == torch.float64:
+            dt = DTYPE_F64
+        elif x.dtype == torch.float32:
+            dt = DTYPE_F32
+        else:
+            raise TypeError(f"{name}: float32 or float64 expected")
+        if not x.is_contiguous():
+            raise ValueError(f"{name}: tensor must be contiguous")
+        return x.data_ptr(), dt, (MEM_DEVICE if x.is_cuda else MEM_HOST), x
+    a = np.asarray(x)
+    if a.dtype == np.float64:
+        dt = DTYPE_F64
+    elif a.dtype == np.float32:
+        dt = DTYPE_F32
+    else:
+        raise TypeError(f"{name}: float32 or float64 expected")
+    if not a.flags.c_contiguous:
+        raise ValueError(f"{name}: array must be C-contiguous")
+    return a.ctypes.data, dt, MEM_HOST, a
+
+
+class Photons:
+    """Thin object wrapper over the C ABI: same calls, same names."""
+
+    def __init__(self, **params):
+        self._lib = load()
+        self._ctx = ctypes.c_void_p()
+        self.params = default_params(**params)
+        buf = ctypes.create_string_buffer(512)
+        rc = self._lib.photons_create(ctypes.byref(self.params), ctypes.byref(self._ctx), buf, len(buf))
+        if rc != OK:
+            self._ctx = ctypes.c_void_p()
+            raise PhotonsError(rc, buf.value.decode(errors="replace"))
+        self.n = 0
+
+    def _check(self, rc):
+        if rc != OK:
+            raise PhotonsError(rc, (self._lib.photons_last_error(self._ctx) or b"").decode(errors="replace"))
+
+    def set_particles(self, pos, mass=None, stream=None):
+        ptr, dt, kind, _keep = _marshal(pos, "pos")
+        n = int(pos.shape[0])
+        if tuple(pos.shape) != (n, 3):
+            raise ValueError("pos must be n x 3")
+        mptr = None
+        if mass is not None:
+            mptr, mdt, mkind, _keepm = _marshal(mass, "mass")
+            if mdt != dt or mkind != kind or tuple(mass.shape) != (n,):
+                raise ValueError("mass must match pos in dtype, memory kind and length")
+        if stream is None and kind == MEM_DEVICE:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(self._lib.photons_set_particles(self._ctx, n, ptr, mptr, dt, kind, ctypes.c_void_p(stream or 0)))
+        self.n = n
+
+    def build_leaves(self):
+        self._check(self._lib.photons_build_leaves(self._ctx))
+
+    def short_range_acc(self, out):
+        """Fill ``out`` (n x 3 numpy array or torch tensor, fp32/fp64, host or device) and return the stats."""
+        ptr, dt, kind, _keep = _marshal(out, "acc")
+        if tuple(out.shape) != (self.n, 3):
+            raise ValueError("acc must be n x 3")
+        if kind == MEM_DEVICE:
+            import torch
+            torch.cuda.current_stream().synchronize()   # the library works on its own streams
+        st = Stats()
+        self._check(self._lib.photons_short_range_acc(self._ctx, ptr, dt, kind, ctypes.byref(st)))
+        return st.as_dict()
+
+    def stats(self):
+        st = Stats()
+        self._check(self._lib.photons_get_stats(self._ctx, ctypes.byref(st)))
+        return st.as_dict()
+
+    def leaf_order(self):
+        st = self.stats()
+        perm = np.empty(st["n_particles"], dtype=np.int64)
+        leaf_start = np.empty(st["n_leaves"] + 1, dtype=np.int64)
+        self._check(self._lib.photons_get_leaf_order(self._ctx, perm.ctypes.data, leaf_start.ctypes.data))
+        return perm, leaf_start
+
+    def interaction_list(self):
+        st = self.stats()
+        ptr = np.empty(st["n_leaves"] + 1, dtype=np.int64)
+        first = np.empty(st["n_chunks"], dtype=np.int32)
+        nleaf = np.empty(st["n_chunks"], dtype=np.int32)
+        code = np.empty(st["n_chunks"], dtype=np.int32)
+        self._check(self._lib.photons_get_interaction_list(self._ctx, ptr.ctypes.data, first.ctypes.data,
+                                                           nleaf.ctypes.data, code.ctypes.data))
+        return ptr, first, nleaf, code
+
+    def close(self):
+        if self._ctx:
+            self._lib.photons_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def peak_probe(kind: int, device: int = 0) -> float:
+    out = ctypes.c_double()
+    rc = load().photons_peak_probe(device, kind, ctypes.byref(out))
+    if rc != OK:
+        raise PhotonsError(rc, "peak_probe failed")
+    return out.value
+
+
+def short_range_acc(pos, mass=None, *, out=None, **params):
+    """One-shot convenience: create -> set_particles -> build_leaves -> short_range_acc -> destroy."""
+    with Photons(**params) as ph:
+        ph.set_particles(pos, mass)
+        ph.build_leaves()
+        if out is None:
+            out = np.empty((pos.shape[0], 3), dtype=np.float64)
+        st = ph.short_range_acc(out)
+    return out, st

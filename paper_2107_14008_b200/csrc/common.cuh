@@ -1,0 +1,116 @@
+// Shared declarations of the photons library (product code; nothing here is used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/photons.h"
+
+namespace photons {
+
+// Interaction-list entry ("chunk"): a run of contiguous source leaves staged as one bulk copy.
+//   .x = first particle slot of the run (leaf * maxleaf)
+//   .y = bits 0..15 number of slots in the run, bits 16..20 shift code 0..26
+//        ((sx+1) + 3 (sy+1) + 9 (sz+1), s = box lengths added to the source) or 27 = per-pair minimum image
+constexpr int SHIFT_NONE = 13;      // code of (0,0,0)
+constexpr int SHIFT_PER_PAIR = 27;  // degenerate geometry: take the minimum image per pair (A10)
+constexpr int N_STAGES = 3;         // shared-memory ring depth per warp
+
+struct GTable {                 // Eq. 2 table
+    int n = 0;                  // intervals over x in [0, 3]; n + 1 nodes
+    int level = 2;
+    float2* d_TE = nullptr;     // {T_i, E_i} per node (fp32)
+    double2* d_TE64 = nullptr;  // fp64 copy for the fp64 path
+};
+
+constexpr int POLY_MAX_DEG = 20;
+
+struct Ctx {
+    photons_params p{};
+    double r_s = 0, r_cut = 0;
+    int sm_count = 0;
+    std::vector<cudaStream_t> streams;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    std::vector<cudaEvent_t> stream_done;
+
+    // particles in caller order (wrapped into [0, L))
+    long long n = 0;
+    double* d_pos = nullptr;   // n x 3
+    double* d_mass = nullptr;  // n
+
+    // ORB / leaves
+    bool leaves_built = false;
+    int depth = 0;              // all leaves at this depth
+    long long n_leaves = 0, n_slots = 0;
+    uint32_t* d_perm = nullptr;     // sorted position -> caller index
+    int* d_slot_src = nullptr;      // slot -> caller index, -1 for padding slots
+    int* d_leaf_cnt = nullptr;      // real particles per leaf
+    double* d_leaf_lo = nullptr;    // n_leaves x 3 tight bbox
+    double* d_leaf_hi = nullptr;
+    double* d_leaf_ctr = nullptr;   // n_leaves x 3 (mixed: origin of the fp32 offsets)
+    double* d_node_lo = nullptr;    // (2 n_leaves - 1) x 3, heap order
+    double* d_node_hi = nullptr;
+    double4* d_p64 = nullptr;       // n_slots x {x, y, z, G m}   (fp64 path and exact close pairs)
+    float* d_p32 = nullptr;         // n_slots/2 x {x0 x1 y0 y1 z0 z1 Gm0 Gm1}  (fp32 / mixed)
+    long long* d_chunk_ptr = nullptr;  // n_leaves + 1
+    uint2* d_chunks = nullptr;
+    int* d_order = nullptr;         // target leaves, heaviest list first
+    long long cap_chunks = 0;
+
+    GTable table;
+    int poly_deg = 0;
+    float poly_c[POLY_MAX_DEG + 1]{};   // Q(s)/(2 r_s)^3 as a polynomial in t = 2 s/s_max - 1, Horner order
+    double poly_err = 0;                // max |g_poly - g| over [0, x_cut] in exact arithmetic
+
+    photons_stats stats{};
+    std::string err;
+};
+
+int fail(Ctx* c, int code, const char* fmt, ...);
+#define PH_CUDA(c, call)                                                                         \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return photons::fail((c), e_ == cudaErrorMemoryAllocation ? PHOTONS_ENOMEM : PHOTONS_ECUDA, \
+                                 "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+// build.cu
+int build_leaves_impl(Ctx* c);
+void free_leaves(Ctx* c);
+// gfunc.cu
+int make_table(Ctx* c);
+int make_poly(Ctx* c);
+// p2p_fp64.cu / p2p_fp32.cu: enqueue the kernel for target leaves order[first .. first+count) on a stream;
+// out = device buffer in caller order (n x 3, fp64 or fp32 as out_f32 says)
+int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st);
+int launch_p2p_fp32(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st);
+
+// first sorted position of segment k at tree level `level` when n particles are bisected with the
+// left child taking floor(size/2) (A13)
+__host__ __device__ inline long long seg_start(long long n, int level, long long k)
+{
+    long long start = 0, size = n;
+    for (int b = level - 1; b >= 0; --b) {
+        long long left = size >> 1;
+        if ((k >> b) & 1) { start += left; size -= left; }
+        else size = left;
+    }
+    return start;
+}
+// segment that holds sorted position q at `level`
+__host__ __device__ inline long long seg_of(long long n, int level, long long q)
+{
+    long long start = 0, size = n, k = 0;
+    for (int b = 0; b < level; ++b) {
+        long long left = size >> 1;
+        k <<= 1;
+        if (q >= start + left) { start += left; size -= left; k |= 1; }
+        else size = left;
+    }
+    return k;
+}
+
+}  // namespace photons

@@ -1,0 +1,55 @@
+// Host side of the fp32 / mixed P2P kernels: argument block, shared-memory sizing, g-mode dispatch.
+#include <cmath>
+
+#include "p2p_fp32_kernel.cuh"
+
+namespace photons {
+
+size_t p32_smem_bytes(Ctx* c, int T)
+{
+    const int W = c->p.warps_per_leaf;
+    size_t b = (size_t)W * N_STAGES * c->p.chunk_max * 16 + (size_t)W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8;
+    if (c->p.g_mode == PHOTONS_G_TABLE) b += (size_t)(c->table.n + 1) * 8;
+    return b;
+}
+
+void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
+{
+    a.p32 = c->d_p32; a.p64 = c->d_p64; a.ctr = c->d_leaf_ctr; a.slot_src = c->d_slot_src;
+    a.chunk_ptr = c->d_chunk_ptr; a.chunks = c->d_chunks; a.order = c->d_order; a.first = first;
+    a.maxleaf = c->p.maxleaf; a.chunk_max = c->p.chunk_max; a.mixed = c->p.precision == PHOTONS_MIXED;
+    a.L = (float)c->p.boxsize; a.invL = (float)(1.0 / c->p.boxsize);
+    a.rcut2 = (float)(c->r_cut * c->r_cut);
+    a.rclose2 = (float)(c->p.close_pair_radius * c->p.close_pair_radius);
+    a.Ld = c->p.boxsize; a.inv2rs_d = 1.0 / (2.0 * c->r_s);
+    // the fast path clamps at the fp32 value of r_close^2; the exact path uses the same radius
+    a.rclose_d = std::sqrt((double)a.rclose2);
+    a.wclose_d = 0.0;
+    if (a.rclose_d > 0) {
+        const double x = a.rclose_d * a.inv2rs_d;
+        const double g = std::erfc(x) + 1.1283791670955125739 * x * std::exp(-x * x);
+        a.wclose_d = g / (a.rclose_d * a.rclose_d * a.rclose_d);
+    }
+    a.inv2rs = (float)a.inv2rs_d;
+    const double smax = 0.25 * c->p.rcut_over_rs * c->p.rcut_over_rs;
+    a.tk = (float)(2.0 / (smax * 4.0 * c->r_s * c->r_s));
+    for (int i = 0; i <= POLY_MAX_DEG; ++i) a.pc[i] = c->poly_c[i];
+    a.tn = c->table.n;
+    a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
+    a.uk = a.tn ? (float)(a.tn / 3.0 * a.inv2rs_d) : 0.f;
+    a.table = c->table.d_TE;
+    a.out = out; a.out_f32 = out_f32 ? 1 : 0;
+}
+
+int launch_p2p_fp32(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st)
+{
+    P32Args a{};
+    fill_p32_args(c, a, first, out, out_f32);
+    switch (c->p.g_mode) {
+        case PHOTONS_G_POLY: return launch_p32_poly(c, a, count, st);
+        case PHOTONS_G_TABLE: return launch_p32_table(c, a, count, st);
+        default: return launch_p32_direct(c, a, count, st);
+    }
+}
+
+}  // namespace photons

@@ -1,0 +1,406 @@
+// fp32 / mixed-precision P2P kernel (Alg. 1 + Alg. 2, the paper's SP run L206), written for sm_100a.
+//
+// Mapping:
+//   CTA            one target leaf (Alg. 1 L96); its W warps split the leaf's source list
+//   lane           T = maxleaf/32 targets in registers (maxleaf 16: the two half-warps take the same 16
+//                  targets and alternate source pairs)
+//   source staging runs of contiguous source leaves, one TMA bulk copy each into a per-warp mbarrier ring
+//   pair core      two sources per lane per step in packed fp32 (add/mul/fma.rn.f32x2 -> FADD2/FMUL2/FFMA2),
+//                  one MUFU.RSQ per pair; sources are read as two broadcast LDS.128 per step
+//   accumulation   fp32 per staged run, flushed into fp64 per-lane sums (two-level, A12)
+//   close pairs    optional: pairs inside close_pair_radius are clamped in the fast path and redone in fp64
+#pragma once
+#include "common.cuh"
+#include "pipeline.cuh"
+
+namespace photons {
+
+constexpr float R2_FLOOR = 1e-24f;       // added to every r^2: self / coincident pairs give w * 0 = 0 (A7)
+constexpr float MAGIC = 12582912.0f;     // 1.5 * 2^23: float -> nearest-integer trick for the table index
+
+struct P32Args {
+    const float* p32;          // n_slots/2 x {x0 x1 y0 y1 z0 z1 Gm0 Gm1}
+    const double4* p64;        // n_slots x {x, y, z, G m}: exact coordinates for the close-pair path
+    const double* ctr;         // n_leaves x 3: origin of each leaf's offsets (MIXED), else unused
+    const int* slot_src;
+    const long long* chunk_ptr;
+    const uint2* chunks;
+    const int* order;
+    long long first;
+    int maxleaf, chunk_max, mixed;
+    float L, invL, rcut2, rclose2;
+    double Ld, inv2rs_d, rclose_d, wclose_d;   // close pairs: g(r_close)/r_close^3 in fp64
+    float inv2rs;              // 1 / 2 r_s
+    float tk;                  // POLY: t = r2 * tk - 1
+    float pc[POLY_MAX_DEG + 1];
+    float uk, h;               // TABLE: u = r * uk in node units, h = 3/n
+    int tn;
+    const float2* table;
+    void* out;
+    int out_f32;
+};
+
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+// one MUFU.RSQ, no denormal fix-up code: r^2 carries R2_FLOOR, so it is never subnormal
+__device__ __forceinline__ float rsq(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+
+// ---------------------------------------------------------------------------------------------------------
+// g-dependent part of the pair core: returns w = G m_j g(r) / r^3 for two pairs at once.
+//   r2   : r^2 (+floor, clamped to r_close^2 when close pairs are on)
+//   gm   : G m_j already multiplied by the cut mask (0 beyond r_cut)
+//   mask : 1 inside r_cut, 0 outside
+// ---------------------------------------------------------------------------------------------------------
+
+template <int DEG>
+__device__ __forceinline__ float2 weight_poly(const P32Args& a, float2 r2, float2 gm, float2 mask)
+{
+    const float2 idr = f2(rsq(r2.x), rsq(r2.y));
+    // masked mapped variable: beyond the cut t = 0 keeps the polynomial bounded
+    float2 t = __ffma2_rn(r2, dup(a.tk), dup(-1.0f));
+    t = __fmul2_rn(t, mask);
+    float2 q = dup(a.pc[0]);
+#pragma unroll
+    for (int k = 1; k <= DEG; ++k) q = __ffma2_rn(q, t, dup(a.pc[k]));
+    const float2 idr2 = __fmul2_rn(idr, idr);
+    const float2 idr3 = __fmul2_rn(idr2, idr);
+    const float2 u = __fadd2_rn(idr3, f2(-q.x, -q.y));      // 1/r^3 - Q(s)/(2 r_s)^3
+    return __fmul2_rn(u, gm);
+}
+
+template <int LEVEL>
+__device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* __restrict__ tab, float2 r2, float2 gm, float2 mask)
+{
+    const float2 idr = f2(rsq(r2.x), rsq(r2.y));
+    // u = x n/3 in node units, 0 beyond the cut (all such lanes then read node 0: a broadcast)
+    float2 u = __fmul2_rn(__fmul2_rn(r2, idr), dup(a.uk));
+    u = __fmul2_rn(u, mask);
+    const float2 um = __fadd2_rn(u, dup(MAGIC));             // nearest node (A14)
+    const float2 fi = __fadd2_rn(um, dup(-MAGIC));
+    const float2 eps = __fmul2_rn(__fadd2_rn(u, f2(-fi.x, -fi.y)), dup(a.h));
+    const float2 xi = __fmul2_rn(fi, dup(a.h));
+    const float2 te0 = tab[__float_as_int(um.x) & 0x1fff];
+    const float2 te1 = tab[__float_as_int(um.y) & 0x1fff];
+    const float2 Ti = f2(te0.x, te1.x), Ei = f2(te0.y, te1.y);
+    float2 T = Ti;
+    if (LEVEL >= 1) {
+        // Eq. 2: T = T_i + E_i eps (x_i^2 - x_i (x_i^2 - 1) eps + (2/3 x_i^4 - 5/3 x_i^2 + 1/3) eps^2 - ...)
+        const float2 xi2 = __fmul2_rn(xi, xi);
+        float2 poly = xi2;
+        if (LEVEL >= 2) {
+            const float2 c2 = __ffma2_rn(f2(-xi.x, -xi.y), xi2, xi);                 // -x_i (x_i^2 - 1)
+            float2 inner = c2;
+            if (LEVEL >= 3) {
+                const float2 c3 = __ffma2_rn(__ffma2_rn(xi2, dup(2.0f / 3.0f), dup(-5.0f / 3.0f)), xi2, dup(1.0f / 3.0f));
+                inner = __ffma2_rn(c3, eps, c2);
+            }
+            poly = __ffma2_rn(inner, eps, xi2);
+        }
+        T = __ffma2_rn(__fmul2_rn(Ei, eps), poly, Ti);
+    }
+    const float2 idr2 = __fmul2_rn(idr, idr);
+    const float2 idr3 = __fmul2_rn(idr2, idr);
+    return __fmul2_rn(__fmul2_rn(idr3, T), gm);
+}
+
+// Eq. 1 by the CUDA library special functions (what the paper's §3.3 L121 calls expensive)
+__device__ __forceinline__ float weight_direct1(const P32Args& a, float r2, float gm)
+{
+    const float idr = rsq(r2);
+    const float x = r2 * idr * a.inv2rs;
+    const float g = erfcf(x) + 1.1283791671f * x * expf(-x * x);
+    return gm * g * (idr * idr * idr);
+}
+
+enum { GM_POLY = 0, GM_TABLE = 1, GM_DIRECT = 2 };
+
+template <int GKIND, int GPAR>
+__device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, float2 r2, float2 gm, float2 mask)
+{
+    if (GKIND == GM_POLY) return weight_poly<GPAR>(a, r2, gm, mask);
+    if (GKIND == GM_TABLE) return weight_table<GPAR>(a, tab, r2, gm, mask);
+    return f2(weight_direct1(a, r2.x, gm.x), weight_direct1(a, r2.y, gm.y));
+}
+
+// exact weight difference for a close pair, fp64: G m_j [g(r)/r^3 - g(r_c)/r_c^3]
+static __device__ __noinline__ double close_pair_weight(double r2, double gm, double inv2rs, double wclose)
+{
+    const double r = sqrt(r2);
+    const double x = r * inv2rs;
+    const double g = erfc(x) + 1.1283791670955125739 * x * exp(-x * x);
+    return gm * (g / (r2 * r) - wclose);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+
+template <int T, bool HALF, int GKIND, int GPAR, bool CLOSE>
+__global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const int M = a.maxleaf;
+    const int stage_bytes = a.chunk_max * 16;
+    unsigned char* ring = smem_raw + (size_t)warp * N_STAGES * stage_bytes;
+    unsigned char* tail = smem_raw + (size_t)W * N_STAGES * stage_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES;
+    uint2* meta = reinterpret_cast<uint2*>(tail + W * N_STAGES * 8) + warp * N_STAGES;
+    double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 16);          // W x T x 32 x 3 doubles
+    float2* tab = reinterpret_cast<float2*>(tail + W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8);
+
+    const long long leaf = a.order[a.first + blockIdx.x];
+    const long long slot0 = leaf * M;
+    const int half = HALF ? lane >> 4 : 0;
+    const int pstep = HALF ? 2 : 1;
+
+    if (GKIND == GM_TABLE) {   // the interpolation table lives in shared memory (Fig. 1)
+        for (int i = threadIdx.x; i <= a.tn; i += blockDim.x) tab[i] = a.table[i];
+        __syncthreads();
+    }
+
+    // targets -> registers (Alg. 1 L99)
+    float tx[T], ty[T], tz[T];
+    double ax[T], ay[T], az[T];
+    int tslot[T];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        const int l = HALF ? (lane & 15) : lane + 32 * t;
+        tslot[t] = (int)slot0 + l;
+        const float* b = a.p32 + (size_t)(tslot[t] >> 1) * 8 + (tslot[t] & 1);
+        tx[t] = b[0]; ty[t] = b[2]; tz[t] = b[4];
+        ax[t] = ay[t] = az[t] = 0.0;
+    }
+    double cix = 0, ciy = 0, ciz = 0;
+    if (a.mixed) { cix = a.ctr[3 * leaf]; ciy = a.ctr[3 * leaf + 1]; ciz = a.ctr[3 * leaf + 2]; }
+
+    const long long c0 = a.chunk_ptr[leaf], c1 = a.chunk_ptr[leaf + 1];
+    const long long n_all = c1 - c0;
+    const int n_my = n_all > warp ? (int)((n_all - warp + W - 1) / W) : 0;
+
+    if (lane == 0) {
+        for (int s = 0; s < N_STAGES; ++s) mbar_init(&bars[s], 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    auto issue = [&](int k) {
+        const uint2 e = a.chunks[c0 + warp + (long long)k * W];
+        const int st = k % N_STAGES;
+        meta[st] = e;
+        const uint32_t bytes = (e.y & 0xffffu) * 16u;
+        mbar_expect_tx(&bars[st], bytes);
+        bulk_g2s(ring + (size_t)st * stage_bytes, a.p32 + (size_t)e.x * 4, bytes, &bars[st]);
+    };
+    if (lane == 0)
+        for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k);
+
+    for (int k = 0; k < n_my; ++k) {
+        const int st = k % N_STAGES;
+        mbar_wait(&bars[st], (uint32_t)(k / N_STAGES) & 1u);
+        const uint2 e = meta[st];
+        const int ns = (int)(e.y & 0xffffu);
+        const int code = (int)((e.y >> 16) & 31u);
+        const float4* src = reinterpret_cast<const float4*>(ring + (size_t)st * stage_bytes);
+        const bool per_pair = code == SHIFT_PER_PAIR;
+        const int sxi = per_pair ? 0 : code % 3 - 1, syi = per_pair ? 0 : (code / 3) % 3 - 1, szi = per_pair ? 0 : code / 9 - 1;
+        // MIXED: every source leaf of the run has its own origin; ABS: one block = the whole run
+        const int blk = a.mixed ? M : ns;
+
+        float px[T], py[T], pz[T];       // fp32 partial sums of this run (level 1 of the accumulation)
+#pragma unroll
+        for (int t = 0; t < T; ++t) px[t] = py[t] = pz[t] = 0.f;
+        float rmin2 = 3.0e38f;
+
+        for (int b0 = 0; b0 < ns; b0 += blk) {
+            // targets as seen from this block: d = (r_j + sadd) - q
+            float qx[T], qy[T], qz[T];
+            float sax = 0.f, say = 0.f, saz = 0.f;
+            if (a.mixed) {
+                const long long jl = (long long)(e.x + b0) / M;
+                const float dcx = (float)((a.ctr[3 * jl] + a.Ld * sxi) - cix);
+                const float dcy = (float)((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy);
+                const float dcz = (float)((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz);
+#pragma unroll
+                for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dcx; qy[t] = ty[t] - dcy; qz[t] = tz[t] - dcz; }
+            } else {
+                // s = +1: move the target by -L (exact, it sits in the upper half of the box);
+                // s = -1: move the sources by -L per pair (exact for the same reason)
+                sax = sxi < 0 ? -a.L : 0.f; say = syi < 0 ? -a.L : 0.f; saz = szi < 0 ? -a.L : 0.f;
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    qx[t] = sxi > 0 ? tx[t] - a.L : tx[t];
+                    qy[t] = syi > 0 ? ty[t] - a.L : ty[t];
+                    qz[t] = szi > 0 ? tz[t] - a.L : tz[t];
+                }
+            }
+            const bool seam = (sax != 0.f) | (say != 0.f) | (saz != 0.f);
+            const float4* s4 = src + b0;             // two float4 per source pair
+            const int np = blk / 2;
+
+            if (per_pair) {
+                // degenerate geometry (tiny N, leaves spanning half the box): minimum image per pair
+                for (int p = half; p < np; p += pstep) {
+                    const float4 A = s4[2 * p], B = s4[2 * p + 1];
+#pragma unroll
+                    for (int t = 0; t < T; ++t) {
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            float dx = (hh ? A.y : A.x) - qx[t], dy = (hh ? A.w : A.z) - qy[t], dz = (hh ? B.y : B.x) - qz[t];
+                            dx -= a.L * rintf(dx * a.invL); dy -= a.L * rintf(dy * a.invL); dz -= a.L * rintf(dz * a.invL);
+                            float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, R2_FLOOR)));
+                            if (CLOSE) { rmin2 = fminf(rmin2, r2); r2 = fmaxf(r2, a.rclose2); }
+                            const float m = r2 < a.rcut2 ? 1.f : 0.f;
+                            const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup((hh ? B.w : B.z) * m), dup(m));
+                            px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
+                        }
+                    }
+                }
+            } else {
+                float2 nqx[T], nqy[T], nqz[T], pax[T], pay[T], paz[T];
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    nqx[t] = dup(-qx[t]); nqy[t] = dup(-qy[t]); nqz[t] = dup(-qz[t]);
+                    pax[t] = pay[t] = paz[t] = dup(0.f);
+                }
+                const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
+                auto step = [&](const float4 A, const float4 B, const bool with_seam) {
+                    float2 xj = f2(A.x, A.y), yj = f2(A.z, A.w), zj = f2(B.x, B.y);
+                    if (with_seam) { xj = __fadd2_rn(xj, sx2); yj = __fadd2_rn(yj, sy2); zj = __fadd2_rn(zj, sz2); }
+#pragma unroll
+                    for (int t = 0; t < T; ++t) {
+                        const float2 dx = __fadd2_rn(xj, nqx[t]), dy = __fadd2_rn(yj, nqy[t]), dz = __fadd2_rn(zj, nqz[t]);
+                        float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __ffma2_rn(dz, dz, dup(R2_FLOOR))));
+                        if (CLOSE) {
+                            rmin2 = fminf(rmin2, fminf(r2.x, r2.y));
+                            r2 = f2(fmaxf(r2.x, a.rclose2), fmaxf(r2.y, a.rclose2));
+                        }
+                        const float2 mask = f2(r2.x < a.rcut2 ? 1.f : 0.f, r2.y < a.rcut2 ? 1.f : 0.f);
+                        const float2 gm = __fmul2_rn(f2(B.z, B.w), mask);
+                        const float2 w = weight2<GKIND, GPAR>(a, tab, r2, gm, mask);
+                        pax[t] = __ffma2_rn(w, dx, pax[t]);
+                        pay[t] = __ffma2_rn(w, dy, pay[t]);
+                        paz[t] = __ffma2_rn(w, dz, paz[t]);
+                    }
+                };
+                if (seam) {
+#pragma unroll 2
+                    for (int p = half; p < np; p += pstep) step(s4[2 * p], s4[2 * p + 1], true);
+                } else {
+#pragma unroll 2
+                    for (int p = half; p < np; p += pstep) step(s4[2 * p], s4[2 * p + 1], false);
+                }
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    px[t] += pax[t].x + pax[t].y; py[t] += pay[t].x + pay[t].y; pz[t] += paz[t].x + paz[t].y;
+                }
+            }
+        }
+        // level 2 of the accumulation: flush the run's fp32 partial sums into the fp64 sums
+#pragma unroll
+        for (int t = 0; t < T; ++t) { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
+
+        if (CLOSE) {
+            // The fast path evaluated pairs inside r_close as if they sat at r_close.  Redo those pairs in
+            // fp64 from the exact coordinates.  Runs that hold the target leaf itself always take this scan
+            // (every lane sees its own r = 0 there); elsewhere it is rare.
+            if (__any_sync(0xffffffffu, rmin2 < a.rclose2)) {
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    const double4 pi = a.p64[tslot[t]];
+                    for (int j = half; j < ns; j += pstep) {
+                        const double4 pj = a.p64[e.x + j];
+                        double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                        if (per_pair) {
+                            dx -= a.Ld * rint(dx / a.Ld); dy -= a.Ld * rint(dy / a.Ld); dz -= a.Ld * rint(dz / a.Ld);
+                        } else {
+                            dx += a.Ld * sxi; dy += a.Ld * syi; dz += a.Ld * szi;
+                        }
+                        const double r2 = dx * dx + dy * dy + dz * dz;
+                        if (r2 > 0.0 && r2 < a.rclose_d * a.rclose_d) {
+                            const double w = close_pair_weight(r2, pj.w, a.inv2rs_d, a.wclose_d);
+                            ax[t] += w * dx; ay[t] += w * dy; az[t] += w * dz;
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0 && k + N_STAGES < n_my) issue(k + N_STAGES);
+    }
+
+    if (HALF) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            ax[t] += __shfl_xor_sync(0xffffffffu, ax[t], 16);
+            ay[t] += __shfl_xor_sync(0xffffffffu, ay[t], 16);
+            az[t] += __shfl_xor_sync(0xffffffffu, az[t], 16);
+        }
+    }
+    // sum the warps' partial accelerations in a fixed order (deterministic), then scatter to caller order
+    if (W > 1) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            double* r = red + ((size_t)(warp * T + t) * 32 + lane) * 3;
+            r[0] = ax[t]; r[1] = ay[t]; r[2] = az[t];
+        }
+        __syncthreads();
+        if (warp != 0) return;
+#pragma unroll
+        for (int t = 0; t < T; ++t)
+            for (int w = 1; w < W; ++w) {
+                const double* r = red + ((size_t)(w * T + t) * 32 + lane) * 3;
+                ax[t] += r[0]; ay[t] += r[1]; az[t] += r[2];
+            }
+    }
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        if (HALF && lane >= 16) continue;
+        const int dst = a.slot_src[tslot[t]];
+        if (dst < 0) continue;
+        if (a.out_f32) {
+            float* o = reinterpret_cast<float*>(a.out) + 3 * (size_t)dst;
+            o[0] = (float)ax[t]; o[1] = (float)ay[t]; o[2] = (float)az[t];
+        } else {
+            double* o = reinterpret_cast<double*>(a.out) + 3 * (size_t)dst;
+            o[0] = ax[t]; o[1] = ay[t]; o[2] = az[t];
+        }
+    }
+}
+
+// host side ------------------------------------------------------------------------------------------------
+void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32);
+size_t p32_smem_bytes(Ctx* c, int T);
+
+template <int GKIND, int GPAR, bool CLOSE>
+static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
+{
+    const int W = c->p.warps_per_leaf;
+    const int M = c->p.maxleaf;
+    const int T = M <= 32 ? 1 : M / 32;
+    const size_t smem = p32_smem_bytes(c, T);
+    void (*kern)(P32Args) = nullptr;
+    if (M == 16) kern = p2p_fp32_kernel<1, true, GKIND, GPAR, CLOSE>;
+    else if (M == 32) kern = p2p_fp32_kernel<1, false, GKIND, GPAR, CLOSE>;
+    else if (M == 64) kern = p2p_fp32_kernel<2, false, GKIND, GPAR, CLOSE>;
+    else kern = p2p_fp32_kernel<4, false, GKIND, GPAR, CLOSE>;
+    PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
+    PH_CUDA(c, cudaGetLastError());
+    return PHOTONS_OK;
+}
+
+template <int GKIND, int GPAR>
+static int launch_p32_close(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
+{
+    return c->p.close_pair_radius > 0 ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
+                                      : launch_p32_shape<GKIND, GPAR, false>(c, a, count, st);
+}
+
+int launch_p32_poly(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
+int launch_p32_table(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
+int launch_p32_direct(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
+
+}  // namespace photons

@@ -1,0 +1,134 @@
+// Throughput micro-benchmarks behind photons_peak_probe (include/photons.h): what the B200 issues per second
+// for the instruction classes of the pair core.  They give the measured roofline denominators of DESIGN.md §7
+// next to the nominal SM-count x lanes x clock figure (PAPER.md L190 quotes its peak the same way).
+#include "common.cuh"
+
+namespace photons {
+
+constexpr int PROBE_ITERS = 4096;
+constexpr int CH = 16;   // independent dependency chains per thread
+
+template <int KIND>
+__global__ void __launch_bounds__(256) probe_kernel(float* out, float a_in, float b_in, int iters)
+{
+    __shared__ float4 sh[64];
+    if (threadIdx.x < 64) sh[threadIdx.x] = make_float4(a_in, b_in, a_in, b_in);
+    __syncthreads();
+    float a = a_in, b = b_in;
+    float x[CH];
+    float2 y[CH / 2];
+    double d[CH / 2];
+#pragma unroll
+    for (int i = 0; i < CH; ++i) x[i] = 1.0f + 0.001f * (threadIdx.x + i);
+#pragma unroll
+    for (int i = 0; i < CH / 2; ++i) { y[i] = make_float2(x[2 * i], x[2 * i + 1]); d[i] = x[i]; }
+    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+    float4 acc4 = make_float4(0, 0, 0, 0);
+    for (int it = 0; it < iters; ++it) {
+        if (KIND == 0) {            // FFMA, three register operands
+#pragma unroll
+            for (int i = 0; i < CH; ++i) x[i] = fmaf(x[i], a, b);
+        } else if (KIND == 1) {     // FFMA2
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], a2, b2);
+        } else if (KIND == 2) {     // DFMA
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) d[i] = fma(d[i], (double)a, (double)b);
+        } else if (KIND == 3) {     // MUFU.RSQ
+#pragma unroll
+            for (int i = 0; i < CH; ++i) x[i] = rsqrtf(x[i]);
+        } else if (KIND == 4) {     // 8 FFMA2 : 2 MUFU.RSQ (the pair core's ratio is about 15 : 2)
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], a2, b2);
+            x[0] = rsqrtf(x[0]);
+            x[1] = rsqrtf(x[1]);
+        } else if (KIND == 5) {     // LDS.128, one address per warp (broadcast)
+#pragma unroll
+            for (int i = 0; i < CH; ++i) {
+                const float4 v = sh[(it + i) & 63];
+                acc4.x += v.x; acc4.y += v.y; acc4.z += v.z; acc4.w += v.w;
+            }
+        } else if (KIND == 6) {     // FFMA with immediate operands
+#pragma unroll
+            for (int i = 0; i < CH; ++i) x[i] = fmaf(x[i], 0.999f, 0.001f);
+        } else if (KIND == 7) {     // 8 FFMA2 : 4 ALU-pipe ops (compare-to-float, min)
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], a2, b2);
+            x[0] = x[0] < a ? 1.f : 0.f;
+            x[1] = fminf(x[1], b);
+            x[2] = x[2] < b ? 1.f : 0.f;
+            x[3] = fmaxf(x[3], a);
+        } else if (KIND == 8) {     // FADD2
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __fadd2_rn(y[i], a2);
+        } else if (KIND == 9) {     // FMUL2
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __fmul2_rn(y[i], a2);
+        } else if (KIND == 10) {    // FFMA2 with both multiplicands distinct per chain (no operand reuse)
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
+        }
+    }
+    float s = acc4.x + acc4.y + acc4.z + acc4.w;
+#pragma unroll
+    for (int i = 0; i < CH; ++i) s += x[i];
+#pragma unroll
+    for (int i = 0; i < CH / 2; ++i) s += y[i].x + y[i].y + (float)d[i];
+    if (s == 123.456f) out[0] = s;   // keeps the chains alive
+}
+
+template <int KIND>
+static cudaError_t run_probe(int sms, float* d_out, float* ms)
+{
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int grid = sms * 8;
+    probe_kernel<KIND><<<grid, 256>>>(d_out, 0.999f, 0.001f, 64);   // warm-up
+    cudaEventRecord(e0);
+    probe_kernel<KIND><<<grid, 256>>>(d_out, 0.999f, 0.001f, PROBE_ITERS);
+    cudaEventRecord(e1);
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaEventElapsedTime(ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return e;
+}
+
+}  // namespace photons
+
+using namespace photons;
+
+extern "C" int photons_peak_probe(int device, int kind, double* out)
+{
+    if (!out || kind < 0 || kind > 10) return PHOTONS_EINVAL;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) {
+        cudaGetLastError();
+        return PHOTONS_ENODEVICE;
+    }
+    float* d_out = nullptr;
+    if (cudaMalloc(&d_out, 16) != cudaSuccess) return PHOTONS_ENOMEM;
+    float ms = 0;
+    cudaError_t e = cudaSuccess;
+    double lane_ops_per_thread_iter = 0;   // FMA = 1 op per lane; f32x2 = 2
+    switch (kind) {
+        case 0: e = run_probe<0>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 1: e = run_probe<1>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 2: e = run_probe<2>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH / 2; break;
+        case 3: e = run_probe<3>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 4: e = run_probe<4>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // counts the FFMA2 lanes only
+        case 5: e = run_probe<5>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // LDS.128 per lane
+        case 6: e = run_probe<6>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 7: e = run_probe<7>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // counts the FFMA2 lanes only
+        case 8: e = run_probe<8>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 9: e = run_probe<9>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        default: e = run_probe<10>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+    }
+    cudaFree(d_out);
+    if (e != cudaSuccess) return PHOTONS_ECUDA;
+    const double threads = (double)prop.multiProcessorCount * 8 * 256;
+    *out = threads * PROBE_ITERS * lane_ops_per_thread_iter / (ms * 1e-3);
+    return PHOTONS_OK;
+}
