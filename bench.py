@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py — the headline measurement of the truncated-P2P hot path on B200 (contract: see DESIGN.md §8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+Metric (BASELINE.json): truncated P2P pair interactions/s (evaluated pairs, the paper's count)
+and the fraction of the B200 FP32 FMA peak, fp32 path.  Workload at N=1: BASELINE config 4 (configs[3]),
+N = 256^3 clustered particles, N_PM = 256, MAXLEAF = 32 — the configuration north_star quotes its target on.
+
+One "step" is one pass of the whole path over the particle set, as the paper's code does once per time step
+(PAPER.md L83-L89): photons_set_particles -> photons_build_leaves (ORB sort, leaf table, interaction list)
+-> photons_short_range_acc (the P2P kernel, output in caller order).
+  value  : evaluated pairs of all ranks / step time, inputs resident in HBM (device pointers)
+  e2e    : the same through the C ABI with HOST buffers: the host->device copy of positions and the
+           device->host copy of the accelerations are inside the timed region
+  roofline: the dominant kernel (p2p_fp32_kernel) alone, CUDA-event time of its launches
+With --gpus N each rank runs an independent replica of the workload (its own seed): the path has no
+cross-rank exchange on one node ("replicas only"), scaling = "weak".
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2107_14008_b200 import workloads  # noqa: E402
+
+METRIC = "truncated P2P pair interactions/s (evaluated pairs, fp32 path)"
+UNIT = "pairs/s"
+
+# B200 FP32 vector peak: SMs x FP32 lanes x 2 flop x max SM clock
+SM_COUNT = 148
+FP32_LANES_PER_SM = 128
+# executed flops per evaluated pair of the headline kernel, FFMA = 2, FADD/FMUL/MUFU = 1, counted from its
+# SASS inner loop: poly g of degree d -> (7 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
+def flops_per_pair(g_mode: str, poly_degree: int = 13) -> float:
+    if g_mode == "poly":
+        return 2.0 * (7 + poly_degree) + 3 + 2 + 1
+    if g_mode == "table":      # 512 nodes, level 2: 9 FFMA + 6 FADD + 12 FMUL + 1 MUFU
+        return 2.0 * 9 + 6 + 12 + 1
+    return 51.0                # direct: the paper's convention; erfcf/expf are not itemised
+PAPER_FLOPS_PER_PAIR = 51.0
+
+
+def geometry(cfg):
+    r_s = 1.2 * cfg.boxsize / cfg.n_pm
+    return r_s, 6.0 * r_s                   # r_cut = 6 r_s (north_star)
+
+
+def headline_params(cfg, **over):
+    """The launch configuration this file times (also used by tests/test_gpu_parity.py at full size)."""
+    _, r_cut = geometry(cfg)
+    p = dict(boxsize=cfg.boxsize, n_pm=cfg.n_pm, G=cfg.G, maxleaf=cfg.maxleaf, precision="fp32", g_mode="poly",
+             close_pair_radius=0.02 * r_cut, n_streams=1)
+    p.update(over)
+    return p
+
+
+# ------------------------------------------------------------------------------------------ helpers
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+            self.th.join(timeout=2)
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        busy = [s for s, p in zip(sm, pw) if p > 0.5 * max(pw)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def aggregate(local_ms: float, local_units: float, dist=None):
+    """Whole-job figures from per-rank ones: time = MAX over ranks, units = SUM over ranks.
+    Works on any torch.distributed backend (NCCL on the GPUs, gloo in the CPU test)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except OSError:
+        return {}
+
+
+def rank_config(cfg, rank: int):
+    """Rank r's replica: the same recipe with its own seed (independent problems, no exchange)."""
+    import dataclasses
+    return cfg if rank == 0 else dataclasses.replace(cfg, seed=cfg.seed + 100_000 * rank)
+
+
+# ----------------------------------------------------------------------------------- reference arm
+
+def oracle_sample(cfg, pos, mass, seconds_target: float, n_threads_hint: int):
+    """Time the oracle as it stands on a bounded sample: a seeded subset of targets against all N sources.
+    Returns (pair tests, within-cut pairs, seconds, n_targets)."""
+    import oracle
+    oracle.build()
+    r_s, r_cut = geometry(cfg)
+    # ~1.3e8 pair tests per second per core (measured on the first run; only sets the sample size)
+    n_t = int(max(64, min(cfg.n, seconds_target * 1.3e8 * n_threads_hint / cfg.n)))
+    tgt = workloads.sample_targets(cfg.n, n_t, cfg.seed)
+    t0 = time.perf_counter()
+    _, cnt = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut, G=cfg.G)
+    dt = time.perf_counter() - t0
+    return cnt["pair_tests"], cnt["pairs_in_cut"], dt, len(tgt)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    cfg = workloads.CONFIGS[args.config]
+    pos, mass = workloads.make(cfg)
+    cores = oracle.num_threads()
+    per_step = max(2.0, min(20.0, 60.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(cfg, pos, mass, per_step, cores)
+    tests = incut = secs = 0.0
+    n_t = 0
+    for _ in range(args.steps):
+        a, b, dt, n_t = oracle_sample(cfg, pos, mass, per_step, cores)
+        tests += a; incut += b; secs += dt
+    value = tests / secs
+    sample = f"{n_t} seeded targets x all {cfg.n} sources per step (fp64 minimum-image direct sum, pair tests counted)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_particles": cfg.n, "n_pm": cfg.n_pm, "maxleaf": cfg.maxleaf,
+                   "note": "CPU oracle; its unit of work is the pair TEST (every target against all N sources)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "within_cut_pairs_per_s": incut / secs},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------- our arm
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2107_14008_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.load()
+
+    cfg0 = workloads.CONFIGS[args.config]
+    cfg = rank_config(cfg0, rank)
+    r_s, r_cut = geometry(cfg)
+    pos, mass = workloads.make(cfg)              # flavour F: positions on the fp32 grid (A20)
+    pos32 = pos.astype(np.float32)               # exact: the caller's data are fp32
+    params = headline_params(cfg, device=local, n_streams=args.streams, g_mode=args.g_mode,
+                             precision=args.precision, maxleaf=args.maxleaf or cfg.maxleaf)
+    if args.no_close:
+        params["close_pair_radius"] = 0.0
+    n = cfg.n
+
+    d_pos = torch.from_numpy(pos32).cuda()
+    d_acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    h_pos = torch.from_numpy(pos32).pin_memory()
+    h_acc = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    stream = torch.cuda.current_stream()
+
+    ph = B.Photons(**params)
+    ph.set_stream(stream)
+
+    def step_device():
+        ph.set_particles(d_pos, None, stream=stream.cuda_stream)
+        ph.build_leaves()
+        return ph.short_range_acc(d_acc)
+
+    def step_host():
+        ph.set_particles(h_pos, None, stream=stream.cuda_stream)
+        ph.build_leaves()
+        return ph.short_range_acc(h_acc)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(step, steps):
+        k_ms, b_ms, st = [], [], None
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = ph.stats()["kernel_launches"]
+        barrier()
+        e0.record(stream)
+        for _ in range(steps):
+            st = step()
+            k_ms.append(st["kernel_ms"]); b_ms.append(st["build_ms"])
+        e1.record(stream)
+        barrier()
+        return e0.elapsed_time(e1), k_ms, b_ms, st, ph.stats()["kernel_launches"] - l0
+
+    for _ in range(args.warmup):
+        step_device()
+    with ClockSampler(local) as clk:
+        ms, k_ms, b_ms, st, launches = timed(step_device, args.steps)
+    pairs = float(st["pairs_evaluated"])
+    ms_max, units = aggregate(ms, pairs * args.steps, dist if world > 1 else None)
+    value = units / (ms_max * 1e-3)
+
+    # end to end through the C ABI with host buffers
+    for _ in range(min(args.warmup, 2)):
+        step_host()
+    e_steps = max(1, min(args.steps, 3))
+    e_ms, _, _, _, _ = timed(step_host, e_steps)
+    e_ms_max, e_units = aggregate(e_ms, pairs * e_steps, dist if world > 1 else None)
+    e2e_value = e_units / (e_ms_max * 1e-3)
+
+    line = None
+    if rank == 0:
+        kernel_ms = float(np.mean(k_ms))
+        fpp = flops_per_pair(args.g_mode)
+        clocks = clk.summary()
+        peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965.0) * 1e6 / 1e12
+        achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
+        roofline = {
+            "bound": "alu", "kernel": "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+            "frac": achieved_tf / peak_tf, "traffic": None,
+            "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); "
+                           "MEASURED_PEAKS.json holds no FP32 vector peak",
+            "flops_per_pair": fpp, "kernel_ms": kernel_ms, "kernel_pairs_per_s": pairs / (kernel_ms * 1e-3),
+            "kernel_share_of_step": kernel_ms / (ms / args.steps),
+            "frac_at_sampled_clock": (achieved_tf / (SM_COUNT * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
+                                      if clocks["sm_mhz"] else None),
+            "paper_convention_tflops": pairs * PAPER_FLOPS_PER_PAIR / (kernel_ms * 1e-3) / 1e12,
+        }
+        # CPU baseline: the oracle on a bounded sample of the same workload, all host cores
+        cpu = None
+        if not args.no_cpu_baseline:
+            import oracle
+            cores = oracle.num_threads()
+            tests, incut, secs, n_t = oracle_sample(cfg, pos, mass, 15.0, cores)
+            cpu = {"value": tests / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"{n_t} seeded targets x all {n} sources, {secs:.1f} s (pair tests counted; "
+                             f"within-cut pairs/s = {incut / secs:.3e})",
+                   "within_cut_pairs_per_s": incut / secs}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if args.precision != "fp64" else "f64", "data": "synthetic",
+            "config": {"workload": cfg0.name, "n_particles": n, "n_pm": cfg.n_pm, "maxleaf": params["maxleaf"],
+                       "precision": args.precision, "g_mode": args.g_mode, "close_pair_radius_over_rcut": 0.0 if args.no_close else 0.02,
+                       "n_streams": args.streams, "input_flavour": "F (fp32-grid positions)",
+                       "l2": "inputs exceed L2 (leaf-sorted particles + interaction list > 126 MB); no flush",
+                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "step": "set_particles + build_leaves + short_range_acc"},
+            "pairs_evaluated_per_step": pairs, "n_leaf_pairs": st["n_leaf_pairs"], "n_chunks": st["n_chunks"],
+            "build_ms": float(np.mean(b_ms)), "kernel_ms": kernel_ms,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_pos.numel() * 4),
+                    "d2h_bytes_per_step": int(h_acc.numel() * 4), "ms_per_step": e_ms_max / e_steps},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+    ph.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line))
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "mixed", "fp64"])
+    ap.add_argument("--g-mode", dest="g_mode", default="poly", choices=["poly", "table", "direct"])
+    ap.add_argument("--maxleaf", type=int, default=0)
+    ap.add_argument("--streams", type=int, default=1)
+    ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.steps < 1 or args.warmup < 0:
+        ap.error("--steps >= 1 and --warmup >= 0")
+    if args.precision == "fp64" and args.g_mode == "poly":
+        args.g_mode = "direct"
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -98,6 +98,8 @@ typedef struct {
     double build_ms;           /* last photons_build_leaves, host wall clock incl. device sync */
     double kernel_ms;          /* last photons_short_range_acc: CUDA-event time of the P2P launches alone */
     double total_ms;           /* last photons_short_range_acc: host wall clock incl. copies and sync */
+    long long kernel_launches; /* kernels of this library launched on ctx since photons_create (the CUB sort and
+                                  scan launches inside photons_build_leaves are library code and not counted) */
 } photons_stats;
 
 /* Fill *p with the paper's defaults: boxsize 1, n_pm 32, rs_over_cell 1.2, rcut_over_rs 6, G 1, maxleaf 32,
@@ -109,9 +111,15 @@ void photons_default_params(photons_params* p);
  * On error *out is untouched and, if err_buf != NULL, a message is written there (err_len bytes). */
 int photons_create(const photons_params* p, photons_ctx** out, char* err_buf, int err_len);
 
+/* Make `cuda_stream` (a cudaStream_t; NULL = back to the context's own stream) the context's main stream:
+ * build_leaves and short_range_acc enqueue on it (extra streams of n_streams > 1 fork from it and join it
+ * again), so events the caller records on that stream bracket the library's device work.  The stream stays
+ * the caller's.  Errors: EINVAL (null ctx). */
+int photons_set_stream(photons_ctx* ctx, void* cuda_stream);
+
 /* Copy n particles in.  pos: n x 3 row-major, mass: n values or NULL (= 1/n each), both of element type
  * dtype (PHOTONS_DTYPE_*), both host or both device memory as tagged.  Positions are wrapped into
- * [0, boxsize).  cuda_stream: a cudaStream_t the device-side copy is ordered after (NULL = default stream);
+ * [0, boxsize).  cuda_stream: a cudaStream_t the device-side copy is enqueued on (NULL = the context's main stream);
  * the call returns after the copy has completed.  Errors: EINVAL (n < 1, or more than 2^31 - 1 particle slots),
  * ENONFINITE, ENOMEM, ECUDA. */
 int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const void* mass, int dtype,

@@ -25,7 +25,7 @@ G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY}
 ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX", "ENONFINITE"]
 
 EXPORTS = [
-    "photons_default_params", "photons_create", "photons_set_particles", "photons_build_leaves",
+    "photons_default_params", "photons_create", "photons_set_stream", "photons_set_particles", "photons_build_leaves",
     "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
     "photons_peak_probe", "photons_last_error", "photons_destroy",
 ]
@@ -47,7 +47,7 @@ class Stats(ctypes.Structure):
         ("n_particles", ctypes.c_longlong), ("n_leaves", ctypes.c_longlong), ("n_chunks", ctypes.c_longlong),
         ("n_leaf_pairs", ctypes.c_longlong), ("pairs_evaluated", ctypes.c_longlong),
         ("max_leaves_per_target", ctypes.c_longlong), ("build_ms", ctypes.c_double),
-        ("kernel_ms", ctypes.c_double), ("total_ms", ctypes.c_double),
+        ("kernel_ms", ctypes.c_double), ("total_ms", ctypes.c_double), ("kernel_launches", ctypes.c_longlong),
     ]
 
     def as_dict(self):
@@ -77,6 +77,8 @@ def load():
     lib.photons_default_params.argtypes = [ctypes.POINTER(Params)]
     lib.photons_create.restype = ci
     lib.photons_create.argtypes = [ctypes.POINTER(Params), ctypes.POINTER(vp), ctypes.c_char_p, ci]
+    lib.photons_set_stream.restype = ci
+    lib.photons_set_stream.argtypes = [vp, vp]
     lib.photons_set_particles.restype = ci
     lib.photons_set_particles.argtypes = [vp, ll, vp, vp, ci, ci, vp]
     lib.photons_build_leaves.restype = ci
@@ -156,6 +158,11 @@ class Photons:
             raise PhotonsError(rc, buf.value.decode(errors="replace"))
         self.n = 0
 
+    def set_stream(self, stream):
+        """Make a CUDA stream (torch.cuda.Stream, raw handle or None) the context's main stream."""
+        handle = getattr(stream, "cuda_stream", stream)
+        self._check(self._lib.photons_set_stream(self._ctx, ctypes.c_void_p(handle or 0)))
+
     def _check(self, rc):
         if rc != OK:
             raise PhotonsError(rc, (self._lib.photons_last_error(self._ctx) or b"").decode(errors="replace"))
@@ -186,7 +193,7 @@ class Photons:
             raise ValueError("acc must be n x 3")
         if kind == MEM_DEVICE:
             import torch
-            torch.cuda.current_stream().synchronize()   # the library works on its own streams
+            torch.cuda.current_stream().synchronize()   # unless set_stream was used the library has its own streams
         st = Stats()
         self._check(self._lib.photons_short_range_acc(self._ctx, ptr, dt, kind, ctypes.byref(st)))
         return st.as_dict()

@@ -161,6 +161,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         ok = ok && cudaStreamCreateWithFlags(&c->streams[i], cudaStreamNonBlocking) == cudaSuccess;
         ok = ok && cudaEventCreateWithFlags(&c->stream_done[i], cudaEventDisableTiming) == cudaSuccess;
     }
+    c->own_stream0 = c->streams[0];
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
     int rc = PHOTONS_OK;
     if (!ok) rc = fail(c, PHOTONS_ECUDA, "stream/event creation failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -172,6 +173,14 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         return rc;
     }
     *out = reinterpret_cast<photons_ctx*>(c);
+    return PHOTONS_OK;
+}
+
+int photons_set_stream(photons_ctx* ctx, void* cuda_stream)
+{
+    Ctx* c = reinterpret_cast<Ctx*>(ctx);
+    if (!c) return PHOTONS_EINVAL;
+    c->streams[0] = cuda_stream ? reinterpret_cast<cudaStream_t>(cuda_stream) : c->own_stream0;
     return PHOTONS_OK;
 }
 
@@ -187,7 +196,7 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     PH_CUDA(c, cudaSetDevice(c->p.device));
     free_leaves(c);
     free_particles(c);
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    cudaStream_t st = cuda_stream ? reinterpret_cast<cudaStream_t>(cuda_stream) : c->streams[0];
     const size_t esz = dtype == PHOTONS_DTYPE_F64 ? 8 : 4;
     PH_CUDA(c, cudaMalloc(&c->d_pos, sizeof(double) * 3 * n));
     PH_CUDA(c, cudaMalloc(&c->d_mass, sizeof(double) * n));
@@ -212,6 +221,7 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
         intake_kernel<double><<<nb, tb, 0, st>>>(n, (const double*)src_pos, (const double*)src_mass, c->p.boxsize, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
     else
         intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
+    ++c->launches;
     int bad = 0;
     cudaError_t e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -286,6 +296,7 @@ int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind
     cudaEventElapsedTime(&ms, c->ev0, c->ev1);
     c->stats.kernel_ms = ms;
     c->stats.total_ms = now_ms() - t0;
+    c->stats.kernel_launches = c->launches;
     if (stats) *stats = c->stats;
     return PHOTONS_OK;
 }
@@ -327,6 +338,7 @@ int photons_get_stats(photons_ctx* ctx, photons_stats* stats)
 {
     Ctx* c = reinterpret_cast<Ctx*>(ctx);
     if (!c || !stats) return PHOTONS_EINVAL;
+    c->stats.kernel_launches = c->launches;
     *stats = c->stats;
     return PHOTONS_OK;
 }
@@ -346,6 +358,7 @@ void photons_destroy(photons_ctx* ctx)
     free_particles(c);
     cudaFree(c->table.d_TE);
     cudaFree(c->table.d_TE64);
+    if (!c->streams.empty()) c->streams[0] = c->own_stream0;
     for (auto s : c->streams) if (s) cudaStreamDestroy(s);
     for (auto e : c->stream_done) if (e) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);

@@ -312,6 +312,7 @@ int build_leaves_impl(Ctx* c)
 
     PH_CUDA_BUILD(cudaMalloc(&c->d_perm, sizeof(uint32_t) * n));
     iota_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, c->d_perm);
+    ++c->launches;
     if (depth > 0) {
         PH_CUDA_BUILD(cudaMalloc(&d_idx2, sizeof(uint32_t) * n));
         PH_CUDA_BUILD(cudaMalloc(&d_keys, sizeof(unsigned long long) * n));
@@ -325,9 +326,13 @@ int build_leaves_impl(Ctx* c)
         for (int level = 0; level < depth; ++level) {
             const long long nseg = 1LL << level;
             fill_int_kernel<<<blocks_for(3 * nseg, tb), tb, 0, st>>>(3 * nseg, d_blo, 0x7fffffff);
+            ++c->launches;
             fill_int_kernel<<<blocks_for(3 * nseg, tb), tb, 0, st>>>(3 * nseg, d_bhi, 0);
+            ++c->launches;
             seg_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, cur, c->d_pos, d_blo, d_bhi);
+            ++c->launches;
             seg_key_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, cur, c->d_pos, d_blo, d_bhi, d_keys);
+            ++c->launches;
             PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(d_tmp, tmp_bytes, d_keys, d_keys2, cur, alt, (int)n, 0, 32 + level, st));
             std::swap(cur, alt);
         }
@@ -351,10 +356,14 @@ int build_leaves_impl(Ctx* c)
         double* leaf_lo = c->d_node_lo + 3 * (n_leaves - 1);
         double* leaf_hi = c->d_node_hi + 3 * (n_leaves - 1);
         leaf_table_kernel<<<blocks_for(n_leaves, 128), 128, 0, st>>>(n, depth, n_leaves, c->d_perm, c->d_pos, c->d_leaf_cnt, leaf_lo, leaf_hi, c->d_leaf_ctr);
+        ++c->launches;
         pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, c->d_perm, c->d_pos, c->d_mass,
                                                             c->d_leaf_ctr, c->d_slot_src, c->d_p64, c->d_p32);
-        for (int level = depth - 1; level >= 0; --level)
+        ++c->launches;
+        for (int level = depth - 1; level >= 0; --level) {
             node_bbox_kernel<<<blocks_for(1LL << level, tb), tb, 0, st>>>(level, c->d_node_lo, c->d_node_hi);
+            ++c->launches;
+        }
     }
 
     // interaction list: count, scan, fill
@@ -369,6 +378,7 @@ int build_leaves_impl(Ctx* c)
     la.node_lo = c->d_node_lo; la.node_hi = c->d_node_hi; la.leaf_cnt = c->d_leaf_cnt;
     la.chunk_ptr = nullptr; la.chunks = nullptr; la.n_chunks_of = d_nch; la.totals = d_tot; la.work_of = d_work;
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
+    ++c->launches;
     {
         size_t scan_bytes = 0;
         PH_CUDA_BUILD(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_nch, c->d_chunk_ptr, (int)(n_leaves + 1), st));
@@ -385,6 +395,7 @@ int build_leaves_impl(Ctx* c)
     PH_CUDA_BUILD(cudaMalloc(&c->d_chunks, sizeof(uint2) * (size_t)std::max<long long>(h_nchunks, 1)));
     la.chunk_ptr = c->d_chunk_ptr; la.chunks = c->d_chunks;
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
+    ++c->launches;
 
     // heaviest-first order of the target leaves
     PH_CUDA_BUILD(cudaMalloc(&c->d_order, sizeof(int) * n_leaves));
@@ -392,6 +403,7 @@ int build_leaves_impl(Ctx* c)
     PH_CUDA_BUILD(cudaMalloc(&d_okeys2, sizeof(unsigned) * n_leaves));
     PH_CUDA_BUILD(cudaMalloc(&d_ovals, sizeof(int) * n_leaves));
     order_keys_kernel<<<blocks_for(n_leaves, tb), tb, 0, st>>>(n_leaves, d_work, d_okeys, d_ovals);
+    ++c->launches;
     {
         size_t sort_bytes = 0;
         PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairsDescending(nullptr, sort_bytes, d_okeys, d_okeys2, d_ovals, c->d_order, (int)n_leaves, 0, 32, st));

@@ -31,7 +31,9 @@ struct Ctx {
     photons_params p{};
     double r_s = 0, r_cut = 0;
     int sm_count = 0;
-    std::vector<cudaStream_t> streams;
+    std::vector<cudaStream_t> streams;   // [0] = main stream (the caller's after photons_set_stream)
+    cudaStream_t own_stream0 = nullptr;  // the stream created for slot 0 (destroyed with the context)
+    long long launches = 0;              // kernels of this library launched so far (cub's are not counted)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     std::vector<cudaEvent_t> stream_done;
 

@@ -388,6 +388,7 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     else kern = p2p_fp32_kernel<4, false, GKIND, GPAR, CLOSE>;
     PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
+    ++c->launches;
     PH_CUDA(c, cudaGetLastError());
     return PHOTONS_OK;
 }

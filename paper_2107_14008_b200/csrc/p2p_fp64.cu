@@ -180,6 +180,7 @@ static int launch_t(Ctx* c, const P64Args& a, long long count, int W, size_t sme
     auto kern = p2p_fp64_kernel<T, GMODE, LEVEL>;
     PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
+    ++c->launches;
     PH_CUDA(c, cudaGetLastError());
     return PHOTONS_OK;
 }
