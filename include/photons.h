@@ -85,7 +85,7 @@ typedef struct {
                                  0 = default (128); multiple of maxleaf, <= 256 */
     int warps_per_leaf;       /* warps of the CTA that owns one target leaf; they split its source list.
                                  0 = default; 1, 2, 4 or 8 */
-    int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (13) */
+    int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12) */
 } photons_params;
 
 typedef struct {
@@ -152,9 +152,18 @@ int photons_get_stats(photons_ctx* ctx, photons_stats* stats);
  * kind 0 = FFMA (register operands), 1 = FFMA2 (fma.rn.f32x2), 2 = DFMA, 3 = MUFU.RSQ,
  * 4 = FFMA2 with 2 MUFU.RSQ per 8 (FFMA2 lanes counted), 5 = LDS.128 broadcast, 6 = FFMA with immediates,
  * 7 = FFMA2 with 4 ALU-pipe ops per 8 (FFMA2 lanes counted), 8 = FADD2, 9 = FMUL2, 10 = FFMA2 without
- * operand reuse.  *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction
+ * operand reuse; 11..15 = the pair core's mix per step, 24 FFMA2 in two dependent chains (14) plus 2 MUFU.RSQ (11),
+ * plus 2 FSETP+FSEL (12), or plus 2 broadcast LDS.128 (13), or plus both (15) — FFMA2 lanes counted.
+ * kind + 100 b (b = 1..7) runs the probe with only b resident blocks of 8 warps per SM.  *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction
  * counts 2 per lane; multiply FMA rates by 2 for flops).  Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
 int photons_peak_probe(int device, int kind, double* out);
+
+/* Host-only (needs no device): the polynomial behind PHOTONS_G_POLY.  With s = (r/2r_s)^2, s_max = (rcut_over_rs/2)^2
+ * and t = 2 s/s_max - 1, the kernels use g(r) ~= 1 - s^(3/2) * sum_k coeffs[k] t^k (derived from the
+ * integral form of T).  coeffs: degree + 1 doubles (output, lowest power first); max_err_g (may be
+ * NULL): largest |approximation - g| over 0 <= r <= r_cut in exact arithmetic.  Errors: EINVAL (degree outside
+ * 1..20, rcut_over_rs outside (0, 6], null coeffs). */
+int photons_poly_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g);
 
 /* Message of the last failing call on ctx; valid until the next call on ctx. */
 const char* photons_last_error(const photons_ctx* ctx);

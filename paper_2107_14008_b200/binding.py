@@ -27,7 +27,7 @@ ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX",
 EXPORTS = [
     "photons_default_params", "photons_create", "photons_set_stream", "photons_set_particles", "photons_build_leaves",
     "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
-    "photons_peak_probe", "photons_last_error", "photons_destroy",
+    "photons_peak_probe", "photons_poly_fit", "photons_last_error", "photons_destroy",
 ]
 
 
@@ -93,6 +93,8 @@ def load():
     lib.photons_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
     lib.photons_peak_probe.restype = ci
     lib.photons_peak_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.photons_poly_fit.restype = ci
+    lib.photons_poly_fit.argtypes = [ci, ctypes.c_double, vp, ctypes.POINTER(ctypes.c_double)]
     lib.photons_last_error.restype = ctypes.c_char_p
     lib.photons_last_error.argtypes = [vp]
     lib.photons_destroy.restype = None
@@ -244,6 +246,16 @@ def peak_probe(kind: int, device: int = 0) -> float:
     if rc != OK:
         raise PhotonsError(rc, "peak_probe failed")
     return out.value
+
+
+def poly_fit(degree: int, rcut_over_rs: float = 6.0):
+    """(coeffs[degree+1] lowest power first, max |g_poly - g|) of the PHOTONS_G_POLY polynomial; host only."""
+    coeffs = np.empty(degree + 1, dtype=np.float64)
+    err = ctypes.c_double()
+    rc = load().photons_poly_fit(degree, float(rcut_over_rs), coeffs.ctypes.data, ctypes.byref(err))
+    if rc != OK:
+        raise PhotonsError(rc, "poly_fit: bad argument")
+    return coeffs, err.value
 
 
 def short_range_acc(pos, mass=None, *, out=None, **params):

@@ -126,7 +126,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.warps_per_leaf == 0) p.warps_per_leaf = 4;
     if (p.warps_per_leaf != 1 && p.warps_per_leaf != 2 && p.warps_per_leaf != 4 && p.warps_per_leaf != 8)
         return create_fail(err_buf, err_len, PHOTONS_EINVAL, "warps_per_leaf must be 1, 2, 4 or 8");
-    if (p.poly_degree == 0) p.poly_degree = 13;
+    if (p.poly_degree == 0) p.poly_degree = 12;
     if (p.poly_degree < 10 || p.poly_degree > 14) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "poly_degree must be 10..14");
 
     const double r_s = p.rs_over_cell * p.boxsize / p.n_pm;

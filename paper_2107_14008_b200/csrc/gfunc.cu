@@ -2,7 +2,7 @@
 //   make_table : the paper's interpolation table {T_i, E_i} (§3.3), built in extended precision
 //                and rounded once;
 //   make_poly  : coefficients of Q(s) = (1 - g(sqrt s)) / s^(3/2), s = (r / 2 r_s)^2, as a polynomial in the
-//                mapped variable t = 2 s / s_max - 1 (Chebyshev interpolation, converted to monomials),
+//                mapped variable t = 2 s / s_max - 1 (weighted minimax fit, converted to monomials),
 //                so that g(r)/r^3 = 1/r^3 - Q(s)/(2 r_s)^3 needs no special function.
 // Nothing here is shared with oracle/.
 #include <cmath>
@@ -53,25 +53,86 @@ static long double Q_of_s(long double s)
     return (1.0L - g) / (x * s);
 }
 
-int make_poly(Ctx* c)
+// Least squares of the M x N system A x = b by Householder QR, in long double (N <= POLY_MAX_DEG + 1).
+static void lstsq(std::vector<long double>& A, std::vector<long double>& b, int M, int N, std::vector<long double>& x)
 {
-    const int deg = c->p.poly_degree;
-    const int N = deg + 1;
-    const long double xcut = 0.5L * c->p.rcut_over_rs;
-    const long double smax = xcut * xcut;
-    // Chebyshev interpolation on N nodes
-    std::vector<long double> f(N), cheb(N);
-    for (int j = 0; j < N; ++j) {
-        const long double t = cosl(PI_L * (j + 0.5L) / N);
-        f[j] = Q_of_s(0.5L * smax * (t + 1.0L));
-    }
     for (int k = 0; k < N; ++k) {
-        long double a = 0;
-        for (int j = 0; j < N; ++j) a += f[j] * cosl(PI_L * k * (j + 0.5L) / N);
-        cheb[k] = (k == 0 ? 1.0L : 2.0L) * a / N;
+        long double norm = 0;
+        for (int i = k; i < M; ++i) norm += A[(size_t)i * N + k] * A[(size_t)i * N + k];
+        norm = sqrtl(norm);
+        if (norm == 0) continue;
+        const long double alpha = A[(size_t)k * N + k] > 0 ? -norm : norm;
+        std::vector<long double> v(M - k);
+        for (int i = k; i < M; ++i) v[i - k] = A[(size_t)i * N + k];
+        v[0] -= alpha;
+        long double vv = 0;
+        for (long double e : v) vv += e * e;
+        if (vv == 0) continue;
+        for (int j = k; j < N; ++j) {
+            long double dot = 0;
+            for (int i = k; i < M; ++i) dot += v[i - k] * A[(size_t)i * N + j];
+            const long double f = 2 * dot / vv;
+            for (int i = k; i < M; ++i) A[(size_t)i * N + j] -= f * v[i - k];
+        }
+        long double dot = 0;
+        for (int i = k; i < M; ++i) dot += v[i - k] * b[i];
+        const long double f = 2 * dot / vv;
+        for (int i = k; i < M; ++i) b[i] -= f * v[i - k];
+    }
+    x.assign(N, 0.0L);
+    for (int k = N - 1; k >= 0; --k) {
+        long double acc = b[k];
+        for (int j = k + 1; j < N; ++j) acc -= A[(size_t)k * N + j] * x[j];
+        x[k] = acc / A[(size_t)k * N + k];
+    }
+}
+
+// mono[k] = coefficient of t^k (k = 0..deg), t = 2 s/s_max - 1, s_max = (rcut_over_rs / 2)^2; returns the
+// largest |g_poly - g| over [0, x_cut] in exact arithmetic
+static long double fit_poly(int deg, long double rcut_over_rs, std::vector<long double>& mono)
+{
+    const int N = deg + 1;
+    const long double xcut = 0.5L * rcut_over_rs;
+    const long double smax = xcut * xcut;
+    // Weighted minimax fit of Q on [0, s_max] in the Chebyshev basis of t = 2 s/s_max - 1: what matters is the
+    // error of g = 1 - x^3 Q, so the residual carries the weight s^(3/2).  Lawson's iteration (repeated
+    // weighted least squares, weights multiplied by the residual) on a Chebyshev-distributed sample; one
+    // degree cheaper than plain Chebyshev interpolation at equal accuracy in g.
+    const int M = 48 * N;
+    std::vector<long double> tt(M), qq(M), wg(M), lw(M, 1.0L), cheb(N, 0.0L);
+    for (int i = 0; i < M; ++i) {
+        tt[i] = cosl(PI_L * (i + 0.5L) / M);
+        const long double s = 0.5L * smax * (tt[i] + 1.0L);
+        qq[i] = Q_of_s(s);
+        wg[i] = s * sqrtl(s);
+    }
+    std::vector<long double> V((size_t)M * N);
+    for (int i = 0; i < M; ++i) {
+        V[(size_t)i * N] = 1.0L;
+        if (N > 1) V[(size_t)i * N + 1] = tt[i];
+        for (int k = 2; k < N; ++k) V[(size_t)i * N + k] = 2.0L * tt[i] * V[(size_t)i * N + k - 1] - V[(size_t)i * N + k - 2];
+    }
+    for (int it = 0; it < 120; ++it) {
+        std::vector<long double> A((size_t)M * N), b(M);
+        for (int i = 0; i < M; ++i) {
+            const long double w = wg[i] * sqrtl(lw[i]);
+            for (int k = 0; k < N; ++k) A[(size_t)i * N + k] = w * V[(size_t)i * N + k];
+            b[i] = w * qq[i];
+        }
+        lstsq(A, b, M, N, cheb);
+        long double sum = 0;
+        for (int i = 0; i < M; ++i) {
+            long double p = 0;
+            for (int k = 0; k < N; ++k) p += cheb[k] * V[(size_t)i * N + k];
+            lw[i] *= fabsl(wg[i] * (p - qq[i]));
+            sum += lw[i];
+        }
+        if (!(sum > 0)) break;
+        for (int i = 0; i < M; ++i) lw[i] = fmaxl(lw[i] / sum, 1e-40L);
     }
     // to monomials in t: T_0 = 1, T_1 = t, T_{k+1} = 2 t T_k - T_{k-1}
-    std::vector<long double> mono(N, 0.0L), Tkm1(N, 0.0L), Tk(N, 0.0L), Tkp1(N, 0.0L);
+    std::vector<long double> Tkm1(N, 0.0L), Tk(N, 0.0L), Tkp1(N, 0.0L);
+    mono.assign(N, 0.0L);
     Tkm1[0] = 1.0L;
     mono[0] += cheb[0];
     if (N > 1) {
@@ -85,10 +146,6 @@ int make_poly(Ctx* c)
         Tkm1 = Tk;
         Tk = Tkp1;
     }
-    // scale by (1/2r_s)^3 and round once; Horner order (highest degree first)
-    const long double k3 = 1.0L / (8.0L * (long double)c->r_s * c->r_s * c->r_s);
-    c->poly_deg = deg;
-    for (int i = 0; i <= deg; ++i) c->poly_c[i] = (float)(mono[deg - i] * k3);
     // truncation error of the polynomial, expressed as an error of g:  |x^3 (P - Q)|
     long double worst = 0;
     for (int i = 0; i <= 4000; ++i) {
@@ -99,8 +156,30 @@ int make_poly(Ctx* c)
         const long double e = fabsl(sqrtl(s) * s * (p - Q_of_s(s)));
         if (e > worst) worst = e;
     }
-    c->poly_err = (double)worst;
+    return worst;
+}
+
+int make_poly(Ctx* c)
+{
+    const int deg = c->p.poly_degree;
+    std::vector<long double> mono;
+    c->poly_err = (double)fit_poly(deg, c->p.rcut_over_rs, mono);
+    // scale by (1/2r_s)^3 and round once; Horner order (highest degree first)
+    const long double k3 = 1.0L / (8.0L * (long double)c->r_s * c->r_s * c->r_s);
+    c->poly_deg = deg;
+    for (int i = 0; i <= deg; ++i) c->poly_c[i] = (float)(mono[deg - i] * k3);
     return PHOTONS_OK;
 }
 
 }  // namespace photons
+
+// Host-only hook (no device needed): the fitted polynomial itself, for checks against an independent g.
+extern "C" int photons_poly_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g)
+{
+    if (degree < 1 || degree > photons::POLY_MAX_DEG || !(rcut_over_rs > 0) || rcut_over_rs > 6.0 || !coeffs) return PHOTONS_EINVAL;
+    std::vector<long double> mono;
+    const long double e = photons::fit_poly(degree, rcut_over_rs, mono);
+    for (int k = 0; k <= degree; ++k) coeffs[k] = (double)mono[k];
+    if (max_err_g) *max_err_g = (double)e;
+    return PHOTONS_OK;
+}

@@ -8,7 +8,7 @@ namespace photons {
 size_t p32_smem_bytes(Ctx* c, int T)
 {
     const int W = c->p.warps_per_leaf;
-    size_t b = (size_t)W * N_STAGES * c->p.chunk_max * 16 + (size_t)W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8;
+    size_t b = (size_t)W * N_STAGES * c->p.chunk_max * 16 + (size_t)W * N_STAGES * 8 + (size_t)W * T * 32 * 3 * 8;
     if (c->p.g_mode == PHOTONS_G_TABLE) b += (size_t)(c->table.n + 1) * 8;
     return b;
 }
@@ -37,6 +37,7 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     a.tn = c->table.n;
     a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
     a.uk = a.tn ? (float)(a.tn / 3.0 * a.inv2rs_d) : 0.f;
+    a.umax = (float)a.tn;
     a.table = c->table.d_TE;
     a.out = out; a.out_f32 = out_f32 ? 1 : 0;
 }

@@ -33,7 +33,7 @@ struct P32Args {
     float inv2rs;              // 1 / 2 r_s
     float tk;                  // POLY: t = r2 * tk - 1
     float pc[POLY_MAX_DEG + 1];
-    float uk, h;               // TABLE: u = r * uk in node units, h = 3/n
+    float uk, h, umax;         // TABLE: u = r * uk in node units, h = 3/n, umax = last node
     int tn;
     const float2* table;
     void* out;
@@ -52,34 +52,33 @@ __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
 
 // ---------------------------------------------------------------------------------------------------------
 // g-dependent part of the pair core: returns w = G m_j g(r) / r^3 for two pairs at once.
-//   r2   : r^2 (+floor, clamped to r_close^2 when close pairs are on)
-//   gm   : G m_j already multiplied by the cut mask (0 beyond r_cut)
-//   mask : 1 inside r_cut, 0 outside
+//   r2 : r^2 (+floor, clamped to r_close^2 when close pairs are on)
+//   gm : G m_j
+// The value is only meaningful inside r_cut: the caller replaces it by 0 beyond the cut with a select
+// (FSEL, ALU pipe), which also discards the Inf/NaN the polynomial can produce far outside its range.
+// Keeping the cut out of the arithmetic saves two FMA-pipe multiplies per pair.
 // ---------------------------------------------------------------------------------------------------------
 
 template <int DEG>
-__device__ __forceinline__ float2 weight_poly(const P32Args& a, float2 r2, float2 gm, float2 mask)
+__device__ __forceinline__ float2 weight_poly(const P32Args& a, float2 r2, float2 gm)
 {
     const float2 idr = f2(rsq(r2.x), rsq(r2.y));
-    // masked mapped variable: beyond the cut t = 0 keeps the polynomial bounded
-    float2 t = __ffma2_rn(r2, dup(a.tk), dup(-1.0f));
-    t = __fmul2_rn(t, mask);
+    const float2 t = __ffma2_rn(r2, dup(a.tk), dup(-1.0f));          // s mapped to [-1, 1]
     float2 q = dup(a.pc[0]);
 #pragma unroll
     for (int k = 1; k <= DEG; ++k) q = __ffma2_rn(q, t, dup(a.pc[k]));
     const float2 idr2 = __fmul2_rn(idr, idr);
-    const float2 idr3 = __fmul2_rn(idr2, idr);
-    const float2 u = __fadd2_rn(idr3, f2(-q.x, -q.y));      // 1/r^3 - Q(s)/(2 r_s)^3
+    const float2 u = __ffma2_rn(idr2, idr, f2(-q.x, -q.y));          // 1/r^3 - Q(s)/(2 r_s)^3
     return __fmul2_rn(u, gm);
 }
 
 template <int LEVEL>
-__device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* __restrict__ tab, float2 r2, float2 gm, float2 mask)
+__device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* __restrict__ tab, float2 r2, float2 gm)
 {
     const float2 idr = f2(rsq(r2.x), rsq(r2.y));
-    // u = x n/3 in node units, 0 beyond the cut (all such lanes then read node 0: a broadcast)
+    // u = x n/3 in node units, clamped to the last node (FMNMX, ALU pipe) so that the index stays in range
     float2 u = __fmul2_rn(__fmul2_rn(r2, idr), dup(a.uk));
-    u = __fmul2_rn(u, mask);
+    u = f2(fminf(u.x, a.umax), fminf(u.y, a.umax));
     const float2 um = __fadd2_rn(u, dup(MAGIC));             // nearest node (A14)
     const float2 fi = __fadd2_rn(um, dup(-MAGIC));
     const float2 eps = __fmul2_rn(__fadd2_rn(u, f2(-fi.x, -fi.y)), dup(a.h));
@@ -120,12 +119,53 @@ __device__ __forceinline__ float weight_direct1(const P32Args& a, float r2, floa
 enum { GM_POLY = 0, GM_TABLE = 1, GM_DIRECT = 2 };
 
 template <int GKIND, int GPAR>
-__device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, float2 r2, float2 gm, float2 mask)
+__device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, float2 r2, float2 gm)
 {
-    if (GKIND == GM_POLY) return weight_poly<GPAR>(a, r2, gm, mask);
-    if (GKIND == GM_TABLE) return weight_table<GPAR>(a, tab, r2, gm, mask);
-    return f2(weight_direct1(a, r2.x, gm.x), weight_direct1(a, r2.y, gm.y));
+    float2 w;
+    if (GKIND == GM_POLY) w = weight_poly<GPAR>(a, r2, gm);
+    else if (GKIND == GM_TABLE) w = weight_table<GPAR>(a, tab, r2, gm);
+    else w = f2(weight_direct1(a, r2.x, gm.x), weight_direct1(a, r2.y, gm.y));
+    // the cut (A8) and, with it, everything the approximations do outside their range
+    return f2(r2.x < a.rcut2 ? w.x : 0.f, r2.y < a.rcut2 ? w.y : 0.f);
 }
+
+// The same for NCH independent chains (targets x unrolled source pairs) at once.  The polynomial is a chain
+// of dependent FFMA2s, one every ~4 clocks per warp; writing the Horner steps of all chains side by side
+// keeps NCH of them in flight, which is what lets a few warps per scheduler saturate the FMA pipe.
+template <int GKIND, int GPAR, int NCH>
+__device__ __forceinline__ void weights(const P32Args& a, const float2* tab, const float2 (&r2)[NCH], const float2 (&gm)[NCH],
+                                        float2 (&w)[NCH])
+{
+    if (GKIND == GM_POLY) {
+        float2 idr[NCH], t[NCH], q[NCH];
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            idr[c] = f2(rsq(r2[c].x), rsq(r2[c].y));
+            t[c] = __ffma2_rn(r2[c], dup(a.tk), dup(-1.0f));
+            q[c] = __ffma2_rn(dup(a.pc[0]), t[c], dup(a.pc[1]));
+        }
+#pragma unroll
+        for (int k = 2; k <= GPAR; ++k) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) q[c] = __ffma2_rn(q[c], t[c], dup(a.pc[k]));
+        }
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
+            const float2 u = __ffma2_rn(idr2, idr[c], f2(-q[c].x, -q[c].y));
+            const float2 v = __fmul2_rn(u, gm[c]);
+            w[c] = f2(r2[c].x < a.rcut2 ? v.x : 0.f, r2[c].y < a.rcut2 ? v.y : 0.f);
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR>(a, tab, r2[c], gm[c]);
+    }
+}
+
+// smallest r^2 seen so far, self / coincident pairs (r^2 == R2_FLOOR exactly) excluded: as unsigned integers
+// the bit patterns of positive floats keep their order, and subtracting bits(R2_FLOOR) + 1 wraps the
+// excluded value to the top (two ALU-pipe integer ops per pair instead of a compare, a select and a min)
+__device__ __forceinline__ unsigned close_key(float r2) { return (unsigned)__float_as_int(r2) - ((unsigned)__float_as_int(R2_FLOOR) + 1u); }
 
 // exact weight difference for a close pair, fp64: G m_j [g(r)/r^3 - g(r_c)/r_c^3]
 static __device__ __noinline__ double close_pair_weight(double r2, double gm, double inv2rs, double wclose)
@@ -148,9 +188,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     unsigned char* ring = smem_raw + (size_t)warp * N_STAGES * stage_bytes;
     unsigned char* tail = smem_raw + (size_t)W * N_STAGES * stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES;
-    uint2* meta = reinterpret_cast<uint2*>(tail + W * N_STAGES * 8) + warp * N_STAGES;
-    double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 16);          // W x T x 32 x 3 doubles
-    float2* tab = reinterpret_cast<float2*>(tail + W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8);
+    double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 8);           // W x T x 32 x 3 doubles
+    float2* tab = reinterpret_cast<float2*>(tail + W * N_STAGES * 8 + (size_t)W * T * 32 * 3 * 8);
 
     const long long leaf = a.order[a.first + blockIdx.x];
     const long long slot0 = leaf * M;
@@ -186,21 +225,35 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         mbar_fence_init();
     }
     __syncwarp();
-    auto issue = [&](int k) {
-        const uint2 e = a.chunks[c0 + warp + (long long)k * W];
-        const int st = k % N_STAGES;
-        meta[st] = e;
-        const uint32_t bytes = (e.y & 0xffffu) * 16u;
-        mbar_expect_tx(&bars[st], bytes);
-        bulk_g2s(ring + (size_t)st * stage_bytes, a.p32 + (size_t)e.x * 4, bytes, &bars[st]);
+    // Interaction-list entries of this warp, 32 at a time in registers (one per lane, coalesced when W == 1)
+    // and one batch ahead, so that neither the producer nor the consumer ever waits on a global load.
+    const uint2* my_chunks = a.chunks + c0 + warp;
+    auto load_batch = [&](int b) {
+        const int idx = b * 32 + lane;
+        return idx < n_my ? __ldg(&my_chunks[(long long)idx * W]) : make_uint2(0u, 0u);
     };
-    if (lane == 0)
-        for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k);
+    uint2 dcur = load_batch(0), dnext = load_batch(1);
+    auto entry = [&](int k, int cur_batch) {
+        const uint2 v = (k >> 5) == cur_batch ? dcur : dnext;       // warp-uniform choice
+        return make_uint2(__shfl_sync(0xffffffffu, v.x, k & 31), __shfl_sync(0xffffffffu, v.y, k & 31));
+    };
+    auto issue = [&](int k, int cur_batch) {
+        const uint2 e = entry(k, cur_batch);
+        if (lane == 0) {
+            const int st = k % N_STAGES;
+            const uint32_t bytes = (e.y & 0xffffu) * 16u;
+            mbar_expect_tx(&bars[st], bytes);
+            bulk_g2s(ring + (size_t)st * stage_bytes, a.p32 + (size_t)e.x * 4, bytes, &bars[st]);
+        }
+    };
+    for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k, 0);
 
     for (int k = 0; k < n_my; ++k) {
         const int st = k % N_STAGES;
+        const int batch = k >> 5;
+        if ((k & 31) == 0 && k > 0) { dcur = dnext; dnext = load_batch(batch + 1); }
+        const uint2 e = entry(k, batch);
         mbar_wait(&bars[st], (uint32_t)(k / N_STAGES) & 1u);
-        const uint2 e = meta[st];
         const int ns = (int)(e.y & 0xffffu);
         const int code = (int)((e.y >> 16) & 31u);
         const float4* src = reinterpret_cast<const float4*>(ring + (size_t)st * stage_bytes);
@@ -212,7 +265,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         float px[T], py[T], pz[T];       // fp32 partial sums of this run (level 1 of the accumulation)
 #pragma unroll
         for (int t = 0; t < T; ++t) px[t] = py[t] = pz[t] = 0.f;
-        float rmin2 = 3.0e38f;
+        unsigned kmin = 0xffffffffu;     // close_key of the closest non-coincident pair of this run
 
         for (int b0 = 0; b0 < ns; b0 += blk) {
             // targets as seen from this block: d = (r_j + sadd) - q
@@ -251,9 +304,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                             float dx = (hh ? A.y : A.x) - qx[t], dy = (hh ? A.w : A.z) - qy[t], dz = (hh ? B.y : B.x) - qz[t];
                             dx -= a.L * rintf(dx * a.invL); dy -= a.L * rintf(dy * a.invL); dz -= a.L * rintf(dz * a.invL);
                             float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, R2_FLOOR)));
-                            if (CLOSE) { rmin2 = fminf(rmin2, r2); r2 = fmaxf(r2, a.rclose2); }
-                            const float m = r2 < a.rcut2 ? 1.f : 0.f;
-                            const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup((hh ? B.w : B.z) * m), dup(m));
+                            if (CLOSE) { kmin = min(kmin, close_key(r2)); r2 = fmaxf(r2, a.rclose2); }
+                            const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
                         }
                     }
@@ -266,31 +318,48 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                     pax[t] = pay[t] = paz[t] = dup(0.f);
                 }
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
-                auto step = [&](const float4 A, const float4 B, const bool with_seam) {
-                    float2 xj = f2(A.x, A.y), yj = f2(A.z, A.w), zj = f2(B.x, B.y);
-                    if (with_seam) { xj = __fadd2_rn(xj, sx2); yj = __fadd2_rn(yj, sy2); zj = __fadd2_rn(zj, sz2); }
+                // U source pairs x T targets = NCH independent chains per iteration
+                constexpr int U = T == 1 ? 2 : 1;
+                constexpr int NCH = U * T;
+                auto step = [&](const int p, const bool with_seam) {
+                    float2 dx[NCH], dy[NCH], dz[NCH], r2[NCH], gm[NCH], w[NCH];
 #pragma unroll
-                    for (int t = 0; t < T; ++t) {
-                        const float2 dx = __fadd2_rn(xj, nqx[t]), dy = __fadd2_rn(yj, nqy[t]), dz = __fadd2_rn(zj, nqz[t]);
-                        float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __ffma2_rn(dz, dz, dup(R2_FLOOR))));
-                        if (CLOSE) {
-                            rmin2 = fminf(rmin2, fminf(r2.x, r2.y));
-                            r2 = f2(fmaxf(r2.x, a.rclose2), fmaxf(r2.y, a.rclose2));
+                    for (int u = 0; u < U; ++u) {
+                        const float4 A = s4[2 * (p + u * pstep)], B = s4[2 * (p + u * pstep) + 1];
+                        float2 xj = f2(A.x, A.y), yj = f2(A.z, A.w), zj = f2(B.x, B.y);
+                        if (with_seam) { xj = __fadd2_rn(xj, sx2); yj = __fadd2_rn(yj, sy2); zj = __fadd2_rn(zj, sz2); }
+#pragma unroll
+                        for (int t = 0; t < T; ++t) {
+                            const int c = u * T + t;
+                            dx[c] = __fadd2_rn(xj, nqx[t]); dy[c] = __fadd2_rn(yj, nqy[t]); dz[c] = __fadd2_rn(zj, nqz[t]);
+                            gm[c] = f2(B.z, B.w);
                         }
-                        const float2 mask = f2(r2.x < a.rcut2 ? 1.f : 0.f, r2.y < a.rcut2 ? 1.f : 0.f);
-                        const float2 gm = __fmul2_rn(f2(B.z, B.w), mask);
-                        const float2 w = weight2<GKIND, GPAR>(a, tab, r2, gm, mask);
-                        pax[t] = __ffma2_rn(w, dx, pax[t]);
-                        pay[t] = __ffma2_rn(w, dy, pay[t]);
-                        paz[t] = __ffma2_rn(w, dz, paz[t]);
+                    }
+#pragma unroll
+                    for (int c = 0; c < NCH; ++c) {
+                        r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(R2_FLOOR))));
+                        if (CLOSE) {
+                            kmin = min(kmin, min(close_key(r2[c].x), close_key(r2[c].y)));
+                            r2[c] = f2(fmaxf(r2[c].x, a.rclose2), fmaxf(r2[c].y, a.rclose2));
+                        }
+                    }
+                    weights<GKIND, GPAR, NCH>(a, tab, r2, gm, w);
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+#pragma unroll
+                        for (int t = 0; t < T; ++t) {
+                            const int c = u * T + t;
+                            pax[t] = __ffma2_rn(w[c], dx[c], pax[t]);
+                            pay[t] = __ffma2_rn(w[c], dy[c], pay[t]);
+                            paz[t] = __ffma2_rn(w[c], dz[c], paz[t]);
+                        }
                     }
                 };
+                // np is a multiple of U * pstep for every leaf size (np = 8 with two half-warps, else >= 16)
                 if (seam) {
-#pragma unroll 2
-                    for (int p = half; p < np; p += pstep) step(s4[2 * p], s4[2 * p + 1], true);
+                    for (int p = half; p < np; p += pstep * U) step(p, true);
                 } else {
-#pragma unroll 2
-                    for (int p = half; p < np; p += pstep) step(s4[2 * p], s4[2 * p + 1], false);
+                    for (int p = half; p < np; p += pstep * U) step(p, false);
                 }
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
@@ -304,9 +373,9 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 
         if (CLOSE) {
             // The fast path evaluated pairs inside r_close as if they sat at r_close.  Redo those pairs in
-            // fp64 from the exact coordinates.  Runs that hold the target leaf itself always take this scan
-            // (every lane sees its own r = 0 there); elsewhere it is rare.
-            if (__any_sync(0xffffffffu, rmin2 < a.rclose2)) {
+            // fp64 from the exact coordinates.  Self pairs do not trigger the scan (close_key), so it runs
+            // only for runs that really hold a close pair.
+            if (__any_sync(0xffffffffu, kmin < close_key(a.rclose2))) {
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     const double4 pi = a.p64[tslot[t]];
@@ -328,7 +397,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             }
         }
         __syncwarp();
-        if (lane == 0 && k + N_STAGES < n_my) issue(k + N_STAGES);
+        if (k + N_STAGES < n_my) issue(k + N_STAGES, batch);
     }
 
     if (HALF) {
@@ -396,7 +465,7 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
 template <int GKIND, int GPAR>
 static int launch_p32_close(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
 {
-    return c->p.close_pair_radius > 0 ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
+    return a.rclose2 > 1e-20f ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
                                       : launch_p32_shape<GKIND, GPAR, false>(c, a, count, st);
 }
 

@@ -67,6 +67,29 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, float a_in, floa
         } else if (KIND == 10) {    // FFMA2 with both multiplicands distinct per chain (no operand reuse)
 #pragma unroll
             for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
+        } else if (KIND >= 11 && KIND <= 15) {
+            // the pair core's instruction mix per step (two pairs per lane): 24 FFMA2-class in two dependent
+            // chains (Horner), plus 11: 2 MUFU.RSQ (single instruction, ftz)   12: + 2 x (FSETP + FSEL)
+            // 13: + 2 broadcast LDS.128 feeding the chains   15: all of them   14: the chains alone
+            float2 c0 = b2, c1 = b2;
+            if (KIND == 13 || KIND == 15) {
+                const float4 v = sh[it & 63], w = sh[(it + 7) & 63];
+                c0 = make_float2(v.x, v.y);
+                c1 = make_float2(w.z, w.w);
+            }
+#pragma unroll
+            for (int r = 0; r < 12; ++r) {
+                y[0] = __ffma2_rn(y[0], a2, c0);
+                y[1] = __ffma2_rn(y[1], a2, c1);
+            }
+            if (KIND != 14) {
+                asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(x[0]));
+                asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(x[1]));
+            }
+            if (KIND == 12 || KIND == 15) {
+                x[2] = x[2] < a ? x[3] : 0.f;
+                x[4] = x[4] < b ? x[5] : 0.f;
+            }
         }
     }
     float s = acc4.x + acc4.y + acc4.z + acc4.w;
@@ -77,16 +100,20 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, float a_in, floa
     if (s == 123.456f) out[0] = s;   // keeps the chains alive
 }
 
+static int g_blocks_per_sm = 8;   // 8 x 256 threads = 16 warps per scheduler; kinds >= 100 use fewer
+
 template <int KIND>
 static cudaError_t run_probe(int sms, float* d_out, float* ms)
 {
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    const int grid = sms * 8;
-    probe_kernel<KIND><<<grid, 256>>>(d_out, 0.999f, 0.001f, 64);   // warm-up
+    const int grid = sms * 8;   // g_blocks_per_sm of them resident per SM (dynamic shared memory limits it)
+    const size_t dyn = g_blocks_per_sm >= 8 ? 0 : (size_t)(200 * 1024 / g_blocks_per_sm - 2048);
+    cudaFuncSetAttribute(probe_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    probe_kernel<KIND><<<grid, 256, dyn>>>(d_out, 0.999f, 0.001f, 64);   // warm-up
     cudaEventRecord(e0);
-    probe_kernel<KIND><<<grid, 256>>>(d_out, 0.999f, 0.001f, PROBE_ITERS);
+    probe_kernel<KIND><<<grid, 256, dyn>>>(d_out, 0.999f, 0.001f, PROBE_ITERS);
     cudaEventRecord(e1);
     cudaError_t e = cudaEventSynchronize(e1);
     if (e == cudaSuccess) e = cudaGetLastError();
@@ -102,7 +129,10 @@ using namespace photons;
 
 extern "C" int photons_peak_probe(int device, int kind, double* out)
 {
-    if (!out || kind < 0 || kind > 10) return PHOTONS_EINVAL;
+    // kind + 100 * b: the same probe with only b (1..7) resident blocks of 8 warps per SM (occupancy sweep)
+    g_blocks_per_sm = 8;
+    if (kind >= 100) { g_blocks_per_sm = kind / 100; kind %= 100; }
+    if (!out || kind < 0 || kind > 15 || g_blocks_per_sm < 1 || g_blocks_per_sm > 8) return PHOTONS_EINVAL;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) {
         cudaGetLastError();
@@ -124,7 +154,12 @@ extern "C" int photons_peak_probe(int device, int kind, double* out)
         case 7: e = run_probe<7>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // counts the FFMA2 lanes only
         case 8: e = run_probe<8>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
         case 9: e = run_probe<9>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
-        default: e = run_probe<10>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 10: e = run_probe<10>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        case 11: e = run_probe<11>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        case 12: e = run_probe<12>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        case 13: e = run_probe<13>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        case 14: e = run_probe<14>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        default: e = run_probe<15>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
     }
     cudaFree(d_out);
     if (e != cudaSuccess) return PHOTONS_ECUDA;
