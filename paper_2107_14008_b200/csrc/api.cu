@@ -21,6 +21,32 @@ int fail(Ctx* c, int code, const char* fmt, ...)
     return code;
 }
 
+void* workspace(Ctx* c, int slot, size_t bytes)
+{
+    DevBuf& b = c->ws[slot];
+    if (bytes == 0) bytes = 16;
+    if (b.cap >= bytes) return b.p;
+    if (b.p) { cudaFree(b.p); b.p = nullptr; b.cap = 0; }
+    const cudaError_t e = cudaMalloc(&b.p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        b.p = nullptr;
+        fail(c, PHOTONS_ENOMEM, "device allocation of %zu bytes failed (workspace slot %d): %s", bytes, slot, cudaGetErrorString(e));
+        return nullptr;
+    }
+    b.cap = bytes;
+    return b.p;
+}
+
+void workspace_free(Ctx* c)
+{
+    for (DevBuf& b : c->ws) {
+        if (b.p) cudaFree(b.p);
+        b.p = nullptr;
+        b.cap = 0;
+    }
+}
+
 static double now_ms()
 {
     using namespace std::chrono;
@@ -59,8 +85,8 @@ __global__ void convert_out_kernel(long long n3, const double* __restrict__ in, 
 
 static void free_particles(Ctx* c)
 {
-    cudaFree(c->d_pos); c->d_pos = nullptr;
-    cudaFree(c->d_mass); c->d_mass = nullptr;
+    c->d_pos = nullptr;     // the buffers stay in the workspace
+    c->d_mass = nullptr;
     c->n = 0;
 }
 
@@ -198,22 +224,23 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     free_particles(c);
     cudaStream_t st = cuda_stream ? reinterpret_cast<cudaStream_t>(cuda_stream) : c->streams[0];
     const size_t esz = dtype == PHOTONS_DTYPE_F64 ? 8 : 4;
-    PH_CUDA(c, cudaMalloc(&c->d_pos, sizeof(double) * 3 * n));
-    PH_CUDA(c, cudaMalloc(&c->d_mass, sizeof(double) * n));
-    void *d_in_pos = nullptr, *d_in_mass = nullptr;
+    c->d_pos = static_cast<double*>(workspace(c, WS_POS, sizeof(double) * 3 * n));
+    c->d_mass = static_cast<double*>(workspace(c, WS_MASS, sizeof(double) * n));
+    int* d_bad = static_cast<int*>(workspace(c, WS_FLAG, sizeof(int)));
+    if (!c->d_pos || !c->d_mass || !d_bad) { free_particles(c); return PHOTONS_ENOMEM; }
     const void *src_pos = pos, *src_mass = mass;
     if (mem_kind == PHOTONS_MEM_HOST) {
-        PH_CUDA(c, cudaMalloc(&d_in_pos, esz * 3 * n));
+        void* d_in_pos = workspace(c, WS_IN_POS, esz * 3 * n);
+        if (!d_in_pos) { free_particles(c); return PHOTONS_ENOMEM; }
         PH_CUDA(c, cudaMemcpyAsync(d_in_pos, pos, esz * 3 * n, cudaMemcpyHostToDevice, st));
         src_pos = d_in_pos;
         if (mass) {
-            PH_CUDA(c, cudaMalloc(&d_in_mass, esz * n));
+            void* d_in_mass = workspace(c, WS_IN_MASS, esz * n);
+            if (!d_in_mass) { free_particles(c); return PHOTONS_ENOMEM; }
             PH_CUDA(c, cudaMemcpyAsync(d_in_mass, mass, esz * n, cudaMemcpyHostToDevice, st));
             src_mass = d_in_mass;
         }
     }
-    int* d_bad = nullptr;
-    PH_CUDA(c, cudaMalloc(&d_bad, sizeof(int)));
     PH_CUDA(c, cudaMemsetAsync(d_bad, 0, sizeof(int), st));
     const int tb = 256;
     const unsigned nb = (unsigned)((n + tb - 1) / tb);
@@ -225,7 +252,6 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     int bad = 0;
     cudaError_t e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(d_bad); cudaFree(d_in_pos); cudaFree(d_in_mass);
     if (e != cudaSuccess) { free_particles(c); return fail(c, PHOTONS_ECUDA, "set_particles: %s", cudaGetErrorString(e)); }
     if (bad) { free_particles(c); return fail(c, PHOTONS_ENONFINITE, "set_particles: NaN or Inf in positions or masses"); }
     c->n = n;
@@ -260,7 +286,10 @@ int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind
     const bool f32 = dtype == PHOTONS_DTYPE_F32;
     const size_t bytes = (f32 ? 4 : 8) * 3 * (size_t)c->n;
     void* d_out = acc;
-    if (mem_kind == PHOTONS_MEM_HOST) PH_CUDA(c, cudaMalloc(&d_out, bytes));
+    if (mem_kind == PHOTONS_MEM_HOST) {
+        d_out = workspace(c, WS_OUT, bytes);
+        if (!d_out) return PHOTONS_ENOMEM;
+    }
 
     // target-leaf batches round-robin over the streams (north_star: "stream concurrency between leaf
     // batches"; "concurrency management").  The order array is heaviest-first, so batch b
@@ -289,7 +318,6 @@ int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind
     if (e == cudaSuccess && mem_kind == PHOTONS_MEM_HOST) e = cudaMemcpyAsync(acc, d_out, bytes, cudaMemcpyDeviceToHost, s0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s0);
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (mem_kind == PHOTONS_MEM_HOST) cudaFree(d_out);
     if (rc != PHOTONS_OK) return rc;
     if (e != cudaSuccess) return fail(c, PHOTONS_ECUDA, "short_range_acc: %s", cudaGetErrorString(e));
     float ms = 0;
@@ -356,6 +384,7 @@ void photons_destroy(photons_ctx* ctx)
     cudaSetDevice(c->p.device);
     free_leaves(c);
     free_particles(c);
+    workspace_free(c);
     cudaFree(c->table.d_TE);
     cudaFree(c->table.d_TE64);
     if (!c->streams.empty()) c->streams[0] = c->own_stream0;

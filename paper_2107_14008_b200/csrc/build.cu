@@ -10,69 +10,36 @@
 
 namespace photons {
 
+// Device buffers live in the context's grow-only workspace (common.cuh): a rebuild with the same particle
+// number allocates nothing.  Dropping the leaves therefore only resets the state.
 void free_leaves(Ctx* c)
 {
-    cudaFree(c->d_perm); c->d_perm = nullptr;
-    cudaFree(c->d_slot_src); c->d_slot_src = nullptr;
-    cudaFree(c->d_leaf_cnt); c->d_leaf_cnt = nullptr;
-    cudaFree(c->d_leaf_lo); c->d_leaf_lo = nullptr;
-    cudaFree(c->d_leaf_hi); c->d_leaf_hi = nullptr;
-    cudaFree(c->d_leaf_ctr); c->d_leaf_ctr = nullptr;
-    cudaFree(c->d_node_lo); c->d_node_lo = nullptr;
-    cudaFree(c->d_node_hi); c->d_node_hi = nullptr;
-    cudaFree(c->d_p64); c->d_p64 = nullptr;
-    cudaFree(c->d_p32); c->d_p32 = nullptr;
-    cudaFree(c->d_chunk_ptr); c->d_chunk_ptr = nullptr;
-    cudaFree(c->d_chunks); c->d_chunks = nullptr;
-    cudaFree(c->d_order); c->d_order = nullptr;
+    c->d_perm = nullptr; c->d_slot_src = nullptr; c->d_leaf_cnt = nullptr; c->d_leaf_ctr = nullptr;
+    c->d_node_lo = c->d_node_hi = nullptr; c->d_p64 = nullptr; c->d_p32 = nullptr;
+    c->d_chunk_ptr = nullptr; c->d_chunks = nullptr; c->d_order = nullptr;
     c->leaves_built = false;
     c->n_leaves = c->n_slots = 0;
 }
 
 // ---------------------------------------------------------------------------------------------- ORB
-// One tree level: every segment (node) is split at its median along the axis of largest extent of
-// its particle bounding box; the left child takes floor(size/2) particles (A13).  Implemented as a
-// stable radix sort of (segment, fp32 coordinate) keys over the whole array.
+// Every tree node is split at its median along the axis of largest extent of its particle bounding box; the
+// left child takes floor(size/2) particles (A13).  Two phases:
+//   A (levels 0 .. L0-1, nodes larger than ORB_CTA_MAX particles): one stable radix sort per level over the
+//     whole array on keys (node, coordinate as a 24-bit fixed-point number inside the node's bbox).  The
+//     particles travel with the sort as float4 {x, y, z, caller index} in current order, so every pass reads
+//     and writes coalesced; the gather that applies the sorted order also reduces the children's bboxes.
+//   B (levels L0 .. depth-1): one CTA per level-L0 node finishes all remaining levels in shared memory
+//     (bitonic sorts on (child node, coordinate, local index) keys).
+// Splitting coordinates are the positions rounded to fp32; ties go either way, which never changes `a`.
 
-__global__ void iota_kernel(long long n, uint32_t* idx)
+constexpr int ORB_CTA_MAX = 4096;   // particles a phase-B CTA holds in shared memory
+constexpr int ORB_CTA_THREADS = 1024;
+
+__global__ void orb_init_kernel(long long n, const double* __restrict__ pos, float4* __restrict__ P)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i < n) idx[i] = (uint32_t)i;
-}
-
-// bounding boxes of the segments of one level, as fp32 bit patterns (positions are >= 0, so the integer
-// order of the bits is the float order)
-__global__ void seg_bbox_kernel(long long n, int level, const uint32_t* __restrict__ idx,
-                                const double* __restrict__ pos, int* __restrict__ lo, int* __restrict__ hi)
-{
-    long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    const bool live = q < n;
-    const long long qq = live ? q : n - 1;
-    const long long seg = seg_of(n, level, qq);
-    const uint32_t src = idx[qq];
-    int v[3];
-    for (int a = 0; a < 3; ++a) v[a] = __float_as_int((float)pos[3 * (size_t)src + a]);
-    // warp-aggregate when the whole warp sits in one segment
-    const long long seg0 = __shfl_sync(0xffffffffu, seg, 0);
-    const bool uniform = __all_sync(0xffffffffu, seg == seg0);
-    if (uniform) {
-        for (int a = 0; a < 3; ++a) {
-            int mn = v[a], mx = v[a];
-            for (int o = 16; o; o >>= 1) {
-                mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
-                mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            }
-            if ((threadIdx.x & 31) == 0) {
-                atomicMin(&lo[3 * seg + a], mn);
-                atomicMax(&hi[3 * seg + a], mx);
-            }
-        }
-    } else if (live) {
-        for (int a = 0; a < 3; ++a) {
-            atomicMin(&lo[3 * seg + a], v[a]);
-            atomicMax(&hi[3 * seg + a], v[a]);
-        }
-    }
+    if (i >= n) return;
+    P[i] = make_float4((float)pos[3 * i], (float)pos[3 * i + 1], (float)pos[3 * i + 2], __int_as_float((int)i));
 }
 
 __global__ void fill_int_kernel(long long n, int* p, int v)
@@ -81,20 +48,127 @@ __global__ void fill_int_kernel(long long n, int* p, int v)
     if (i < n) p[i] = v;
 }
 
-__global__ void seg_key_kernel(long long n, int level, const uint32_t* __restrict__ idx,
-                               const double* __restrict__ pos, const int* __restrict__ lo,
-                               const int* __restrict__ hi, unsigned long long* __restrict__ keys)
+// P_out[q] = P_in[src[q]] (src == nullptr: identity), and the bounding boxes of the level-`level` nodes as
+// fp32 bit patterns (positions are >= 0, so the integer order of the bits is the float order)
+__global__ void orb_gather_bbox_kernel(long long n, int level, const uint32_t* __restrict__ src,
+                                       const float4* __restrict__ P_in, float4* __restrict__ P_out,
+                                       int* __restrict__ lo, int* __restrict__ hi)
+{
+    long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const bool live = q < n;
+    const long long qq = live ? q : n - 1;
+    const float4 p = src ? P_in[src[qq]] : P_in[qq];
+    if (live && P_out) P_out[q] = p;
+    if (!lo) return;
+    const long long seg = seg_of(n, level, qq);
+    const int v[3] = {__float_as_int(p.x), __float_as_int(p.y), __float_as_int(p.z)};
+    // warp-aggregate when the whole warp sits in one node
+    const long long seg0 = __shfl_sync(0xffffffffu, seg, 0);
+    if (__all_sync(0xffffffffu, seg == seg0)) {
+        for (int a = 0; a < 3; ++a) {
+            const int mn = __reduce_min_sync(0xffffffffu, v[a]), mx = __reduce_max_sync(0xffffffffu, v[a]);
+            if ((threadIdx.x & 31) == 0) { atomicMin(&lo[3 * seg + a], mn); atomicMax(&hi[3 * seg + a], mx); }
+        }
+    } else if (live) {
+        for (int a = 0; a < 3; ++a) { atomicMin(&lo[3 * seg + a], v[a]); atomicMax(&hi[3 * seg + a], v[a]); }
+    }
+}
+
+__device__ __forceinline__ int widest_axis(const float ext[3])
+{
+    int axis = 0;                                   // largest extent, ties -> lowest axis
+    if (ext[1] > ext[axis]) axis = 1;
+    if (ext[2] > ext[axis]) axis = 2;
+    return axis;
+}
+
+__global__ void orb_key_kernel(long long n, int level, const float4* __restrict__ P, const int* __restrict__ lo,
+                               const int* __restrict__ hi, unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals)
 {
     long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (q >= n) return;
     const long long seg = seg_of(n, level, q);
-    float ext[3];
-    for (int a = 0; a < 3; ++a) ext[a] = __int_as_float(hi[3 * seg + a]) - __int_as_float(lo[3 * seg + a]);
-    int axis = 0;                                   // largest extent, ties -> lowest axis
-    if (ext[1] > ext[axis]) axis = 1;
-    if (ext[2] > ext[axis]) axis = 2;
-    const float x = (float)pos[3 * (size_t)idx[q] + axis];
-    keys[q] = ((unsigned long long)seg << 32) | (unsigned long long)(uint32_t)__float_as_int(x);
+    float l[3], ext[3];
+    for (int a = 0; a < 3; ++a) { l[a] = __int_as_float(lo[3 * seg + a]); ext[a] = __int_as_float(hi[3 * seg + a]) - l[a]; }
+    const int axis = widest_axis(ext);
+    const float4 p = P[q];
+    const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
+    // monotone map of [lo, hi] onto 24-bit integers
+    const float u = ext[axis] > 0.f ? (x - l[axis]) / ext[axis] : 0.f;
+    const unsigned f = (unsigned)fminf(u * 16777215.0f, 16777215.0f);
+    keys[q] = ((unsigned long long)seg << 24) | f;
+    vals[q] = (uint32_t)q;
+}
+
+__device__ __forceinline__ void cta_bitonic_sort(unsigned long long* key, int n2)
+{
+    for (int k = 2; k <= n2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < n2; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const unsigned long long a = key[i], b = key[l];
+                    const bool up = (i & k) == 0;
+                    if ((a > b) == up) { key[i] = b; key[l] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// Phase B: CTA b owns the level-L0 node b, sorted positions [seg_start(L0, b), seg_start(L0, b + 1)).
+__global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, int L0, int depth, const float4* __restrict__ P,
+                                                                  uint32_t* __restrict__ perm)
+{
+    extern __shared__ __align__(16) unsigned char orb_smem[];
+    const long long s0 = seg_start(n, L0, blockIdx.x);
+    const long long s1 = blockIdx.x + 1 == (1LL << L0) ? n : seg_start(n, L0, blockIdx.x + 1);
+    const int size = (int)(s1 - s0);
+    int n2 = 1;
+    while (n2 < size) n2 <<= 1;
+    unsigned long long* key = reinterpret_cast<unsigned long long*>(orb_smem);     // ORB_CTA_MAX
+    float4* cur = reinterpret_cast<float4*>(key + ORB_CTA_MAX);                    // ORB_CTA_MAX
+    int* blo = reinterpret_cast<int*>(cur + ORB_CTA_MAX);                          // 3 * 128
+    int* bhi = blo + 3 * 128;
+    for (int e = threadIdx.x; e < size; e += blockDim.x) cur[e] = P[s0 + e];
+    __syncthreads();
+    for (int level = L0; level < depth; ++level) {
+        const int sl = level - L0;                   // nodes of this CTA at this level: 2^sl (<= 128)
+        const int nsub = 1 << sl;
+        for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { blo[i] = 0x7fffffff; bhi[i] = 0; }
+        __syncthreads();
+        for (int e = threadIdx.x; e < size; e += blockDim.x) {
+            const int sub = (int)seg_of(size, sl, e);
+            const float4 p = cur[e];
+            atomicMin(&blo[3 * sub], __float_as_int(p.x)); atomicMax(&bhi[3 * sub], __float_as_int(p.x));
+            atomicMin(&blo[3 * sub + 1], __float_as_int(p.y)); atomicMax(&bhi[3 * sub + 1], __float_as_int(p.y));
+            atomicMin(&blo[3 * sub + 2], __float_as_int(p.z)); atomicMax(&bhi[3 * sub + 2], __float_as_int(p.z));
+        }
+        __syncthreads();
+        for (int e = threadIdx.x; e < n2; e += blockDim.x) {
+            unsigned long long k = ~0ULL;            // padding sorts to the end
+            if (e < size) {
+                const int sub = (int)seg_of(size, sl, e);
+                float ext[3];
+                for (int a = 0; a < 3; ++a) ext[a] = __int_as_float(bhi[3 * sub + a]) - __int_as_float(blo[3 * sub + a]);
+                const int axis = widest_axis(ext);
+                const float4 p = cur[e];
+                const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
+                k = ((unsigned long long)sub << 44) | ((unsigned long long)(unsigned)__float_as_int(x) << 12) | (unsigned)e;
+            }
+            key[e] = k;
+        }
+        __syncthreads();
+        cta_bitonic_sort(key, n2);
+        // apply the order: read through the sorted local indices, then write back
+        float4 tmp[ORB_CTA_MAX / ORB_CTA_THREADS];
+        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) tmp[r] = cur[(int)(key[e] & 0xfffu)];
+        __syncthreads();
+        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) cur[e] = tmp[r];
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < size; e += blockDim.x) perm[s0 + e] = (uint32_t)__float_as_int(cur[e].w);
 }
 
 // ------------------------------------------------------------------------------ leaf table + packing
@@ -269,21 +343,86 @@ __global__ void order_keys_kernel(long long n_leaves, const long long* __restric
 
 // -------------------------------------------------------------------------------------------- driver
 
+__global__ void orb_perm_kernel(long long n, const float4* __restrict__ P, uint32_t* __restrict__ perm)
+{
+    long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (q < n) perm[q] = (uint32_t)__float_as_int(P[q].w);
+}
+
 #define PH_CUDA_BUILD(call)                                                                                 \
     do {                                                                                                    \
         cudaError_t e_ = (call);                                                                            \
-        if (e_ != cudaSuccess) {                                                                            \
-            rc = fail(c, e_ == cudaErrorMemoryAllocation ? PHOTONS_ENOMEM : PHOTONS_ECUDA, "%s:%d %s: %s", \
-                      __FILE__, __LINE__, #call, cudaGetErrorString(e_));                                   \
-            goto done;                                                                                      \
-        }                                                                                                   \
+        if (e_ != cudaSuccess)                                                                              \
+            return fail(c, e_ == cudaErrorMemoryAllocation ? PHOTONS_ENOMEM : PHOTONS_ECUDA, "%s:%d %s: %s", \
+                        __FILE__, __LINE__, #call, cudaGetErrorString(e_));                                 \
+    } while (0)
+#define PH_WS(ptr, type, slot, count)                                                              \
+    do {                                                                                           \
+        (ptr) = static_cast<type*>(workspace(c, (slot), sizeof(type) * (size_t)(count)));          \
+        if (!(ptr)) return PHOTONS_ENOMEM;                                                         \
     } while (0)
 
 static inline unsigned blocks_for(long long n, int tb) { return (unsigned)((n + tb - 1) / tb); }
 
+static int orb_sort(Ctx* c, int depth, cudaStream_t st)
+{
+    const long long n = c->n;
+    const int tb = 256;
+    int L0 = 0;
+    while (L0 < depth && ((n + (1LL << L0) - 1) >> L0) > ORB_CTA_MAX) ++L0;
+    float4 *P_cur = nullptr, *P_alt = nullptr;
+    PH_WS(P_cur, float4, WS_ORB_P0, n);
+    orb_init_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, c->d_pos, P_cur);
+    ++c->launches;
+    if (L0 > 0) {
+        unsigned long long *keys = nullptr, *keys2 = nullptr;
+        uint32_t *vals = nullptr, *vals2 = nullptr;
+        int *lo = nullptr, *hi = nullptr;
+        PH_WS(P_alt, float4, WS_ORB_P1, n);
+        PH_WS(keys, unsigned long long, WS_ORB_KEYS, n);
+        PH_WS(keys2, unsigned long long, WS_ORB_KEYS2, n);
+        PH_WS(vals, uint32_t, WS_ORB_VALS, n);
+        PH_WS(vals2, uint32_t, WS_ORB_VALS2, n);
+        PH_WS(lo, int, WS_ORB_LO, 3LL << L0);
+        PH_WS(hi, int, WS_ORB_HI, 3LL << L0);
+        size_t tmp_bytes = 0;
+        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + L0, st));
+        void* tmp = workspace(c, WS_CUB_TMP, tmp_bytes);
+        if (!tmp) return PHOTONS_ENOMEM;
+        fill_int_kernel<<<1, 32, 0, st>>>(3, lo, 0x7fffffff);
+        fill_int_kernel<<<1, 32, 0, st>>>(3, hi, 0);
+        orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, 0, nullptr, P_cur, nullptr, lo, hi);
+        c->launches += 3;
+        for (int level = 0; level < L0; ++level) {
+            orb_key_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, keys, vals);
+            ++c->launches;
+            PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + level, st));
+            const bool more = level + 1 < L0;   // the next level's boxes, reduced while the order is applied
+            if (more) {
+                const long long nb = 3LL << (level + 1);
+                fill_int_kernel<<<blocks_for(nb, tb), tb, 0, st>>>(nb, lo, 0x7fffffff);
+                fill_int_kernel<<<blocks_for(nb, tb), tb, 0, st>>>(nb, hi, 0);
+                c->launches += 2;
+            }
+            orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level + 1, vals2, P_cur, P_alt, more ? lo : nullptr, hi);
+            ++c->launches;
+            std::swap(P_cur, P_alt);
+        }
+    }
+    if (depth > L0) {
+        const size_t smem = (size_t)ORB_CTA_MAX * (8 + 16) + 2 * 3 * 128 * sizeof(int);
+        PH_CUDA_BUILD(cudaFuncSetAttribute(orb_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        orb_cta_kernel<<<(unsigned)(1LL << L0), ORB_CTA_THREADS, smem, st>>>(n, L0, depth, P_cur, c->d_perm);
+    } else {
+        orb_perm_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, P_cur, c->d_perm);
+    }
+    ++c->launches;
+    PH_CUDA_BUILD(cudaGetLastError());
+    return PHOTONS_OK;
+}
+
 int build_leaves_impl(Ctx* c)
 {
-    int rc = PHOTONS_OK;
     const long long n = c->n;
     const int M = c->p.maxleaf;
     int depth = 0;
@@ -293,73 +432,32 @@ int build_leaves_impl(Ctx* c)
     const long long n_nodes = 2 * n_leaves - 1;
     const int tb = 256;
     cudaStream_t st = c->streams[0];
-
-    // scratch (freed at the end)
-    uint32_t* d_idx2 = nullptr;
-    unsigned long long *d_keys = nullptr, *d_keys2 = nullptr;
-    int *d_blo = nullptr, *d_bhi = nullptr;
-    void* d_tmp = nullptr;
-    size_t tmp_bytes = 0;
-    long long *d_nch = nullptr, *d_work = nullptr;
-    unsigned long long* d_tot = nullptr;
-    unsigned *d_okeys = nullptr, *d_okeys2 = nullptr;
-    int* d_ovals = nullptr;
-    unsigned long long h_tot[2] = {0, 0};
-    long long h_nchunks = 0, h_last = 0;
-    ListArgs la{};
-
     if (n_slots >= (1LL << 31)) return fail(c, PHOTONS_EINVAL, "build_leaves: more than 2^31 particle slots");
+    if (depth - 7 > 24) return fail(c, PHOTONS_EINVAL, "build_leaves: tree too deep");
 
-    PH_CUDA_BUILD(cudaMalloc(&c->d_perm, sizeof(uint32_t) * n));
-    iota_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, c->d_perm);
-    ++c->launches;
-    if (depth > 0) {
-        PH_CUDA_BUILD(cudaMalloc(&d_idx2, sizeof(uint32_t) * n));
-        PH_CUDA_BUILD(cudaMalloc(&d_keys, sizeof(unsigned long long) * n));
-        PH_CUDA_BUILD(cudaMalloc(&d_keys2, sizeof(unsigned long long) * n));
-        PH_CUDA_BUILD(cudaMalloc(&d_blo, sizeof(int) * 3 * (n_leaves / 2)));
-        PH_CUDA_BUILD(cudaMalloc(&d_bhi, sizeof(int) * 3 * (n_leaves / 2)));
-        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, d_keys, d_keys2, c->d_perm, d_idx2, (int)n, 0, 64, st));
-        PH_CUDA_BUILD(cudaMalloc(&d_tmp, tmp_bytes));
-        uint32_t* cur = c->d_perm;
-        uint32_t* alt = d_idx2;
-        for (int level = 0; level < depth; ++level) {
-            const long long nseg = 1LL << level;
-            fill_int_kernel<<<blocks_for(3 * nseg, tb), tb, 0, st>>>(3 * nseg, d_blo, 0x7fffffff);
-            ++c->launches;
-            fill_int_kernel<<<blocks_for(3 * nseg, tb), tb, 0, st>>>(3 * nseg, d_bhi, 0);
-            ++c->launches;
-            seg_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, cur, c->d_pos, d_blo, d_bhi);
-            ++c->launches;
-            seg_key_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, cur, c->d_pos, d_blo, d_bhi, d_keys);
-            ++c->launches;
-            PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(d_tmp, tmp_bytes, d_keys, d_keys2, cur, alt, (int)n, 0, 32 + level, st));
-            std::swap(cur, alt);
-        }
-        if (cur != c->d_perm) {   // keep the result in the buffer the context owns
-            std::swap(c->d_perm, d_idx2);
-        }
-    }
+    PH_WS(c->d_perm, uint32_t, WS_PERM, n);
+    int rc = orb_sort(c, depth, st);
+    if (rc != PHOTONS_OK) return rc;
 
     c->depth = depth;
     c->n_leaves = n_leaves;
     c->n_slots = n_slots;
-    PH_CUDA_BUILD(cudaMalloc(&c->d_leaf_cnt, sizeof(int) * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_node_lo, sizeof(double) * 3 * n_nodes));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_node_hi, sizeof(double) * 3 * n_nodes));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_leaf_ctr, sizeof(double) * 3 * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_slot_src, sizeof(int) * n_slots));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_p64, sizeof(double4) * n_slots));
-    if (c->p.precision != PHOTONS_FP64) PH_CUDA_BUILD(cudaMalloc(&c->d_p32, sizeof(float) * 4 * n_slots));
+    PH_WS(c->d_leaf_cnt, int, WS_LEAF_CNT, n_leaves);
+    PH_WS(c->d_node_lo, double, WS_NODE_LO, 3 * n_nodes);
+    PH_WS(c->d_node_hi, double, WS_NODE_HI, 3 * n_nodes);
+    PH_WS(c->d_leaf_ctr, double, WS_LEAF_CTR, 3 * n_leaves);
+    PH_WS(c->d_slot_src, int, WS_SLOT_SRC, n_slots);
+    PH_WS(c->d_p64, double4, WS_P64, n_slots);
+    c->d_p32 = nullptr;
+    if (c->p.precision != PHOTONS_FP64) PH_WS(c->d_p32, float, WS_P32, 4 * n_slots);
     {
         // the leaves' bboxes are the last n_leaves nodes of the heap arrays
         double* leaf_lo = c->d_node_lo + 3 * (n_leaves - 1);
         double* leaf_hi = c->d_node_hi + 3 * (n_leaves - 1);
         leaf_table_kernel<<<blocks_for(n_leaves, 128), 128, 0, st>>>(n, depth, n_leaves, c->d_perm, c->d_pos, c->d_leaf_cnt, leaf_lo, leaf_hi, c->d_leaf_ctr);
-        ++c->launches;
         pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, c->d_perm, c->d_pos, c->d_mass,
                                                             c->d_leaf_ctr, c->d_slot_src, c->d_p64, c->d_p32);
-        ++c->launches;
+        c->launches += 2;
         for (int level = depth - 1; level >= 0; --level) {
             node_bbox_kernel<<<blocks_for(1LL << level, tb), tb, 0, st>>>(level, c->d_node_lo, c->d_node_hi);
             ++c->launches;
@@ -367,12 +465,15 @@ int build_leaves_impl(Ctx* c)
     }
 
     // interaction list: count, scan, fill
-    PH_CUDA_BUILD(cudaMalloc(&d_nch, sizeof(long long) * (n_leaves + 1)));
-    PH_CUDA_BUILD(cudaMalloc(&d_work, sizeof(long long) * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&d_tot, sizeof(unsigned long long) * 2));
+    long long *d_nch = nullptr, *d_work = nullptr;
+    unsigned long long* d_tot = nullptr;
+    PH_WS(d_nch, long long, WS_LIST_NCH, n_leaves + 1);
+    PH_WS(d_work, long long, WS_LIST_WORK, n_leaves);
+    PH_WS(d_tot, unsigned long long, WS_LIST_TOT, 2);
+    PH_WS(c->d_chunk_ptr, long long, WS_CHUNK_PTR, n_leaves + 1);
     PH_CUDA_BUILD(cudaMemsetAsync(d_tot, 0, sizeof(unsigned long long) * 2, st));
     PH_CUDA_BUILD(cudaMemsetAsync(d_nch, 0, sizeof(long long) * (n_leaves + 1), st));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_chunk_ptr, sizeof(long long) * (n_leaves + 1)));
+    ListArgs la{};
     la.n_leaves = n_leaves; la.depth = depth; la.maxleaf = M; la.chunk_max = c->p.chunk_max;
     la.L = c->p.boxsize; la.rcut = c->r_cut;
     la.node_lo = c->d_node_lo; la.node_hi = c->d_node_hi; la.leaf_cnt = c->d_leaf_cnt;
@@ -382,38 +483,37 @@ int build_leaves_impl(Ctx* c)
     {
         size_t scan_bytes = 0;
         PH_CUDA_BUILD(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_nch, c->d_chunk_ptr, (int)(n_leaves + 1), st));
-        if (scan_bytes > tmp_bytes) {
-            cudaFree(d_tmp); d_tmp = nullptr;
-            PH_CUDA_BUILD(cudaMalloc(&d_tmp, scan_bytes));
-            tmp_bytes = scan_bytes;
-        }
-        PH_CUDA_BUILD(cub::DeviceScan::ExclusiveSum(d_tmp, scan_bytes, d_nch, c->d_chunk_ptr, (int)(n_leaves + 1), st));
+        void* tmp = workspace(c, WS_CUB_TMP, scan_bytes);
+        if (!tmp) return PHOTONS_ENOMEM;
+        PH_CUDA_BUILD(cub::DeviceScan::ExclusiveSum(tmp, scan_bytes, d_nch, c->d_chunk_ptr, (int)(n_leaves + 1), st));
     }
+    unsigned long long h_tot[2] = {0, 0};
+    long long h_nchunks = 0;
     PH_CUDA_BUILD(cudaMemcpyAsync(&h_nchunks, c->d_chunk_ptr + n_leaves, sizeof(long long), cudaMemcpyDeviceToHost, st));
     PH_CUDA_BUILD(cudaMemcpyAsync(h_tot, d_tot, sizeof h_tot, cudaMemcpyDeviceToHost, st));
     PH_CUDA_BUILD(cudaStreamSynchronize(st));
-    PH_CUDA_BUILD(cudaMalloc(&c->d_chunks, sizeof(uint2) * (size_t)std::max<long long>(h_nchunks, 1)));
+    PH_WS(c->d_chunks, uint2, WS_CHUNKS, std::max<long long>(h_nchunks, 1));
     la.chunk_ptr = c->d_chunk_ptr; la.chunks = c->d_chunks;
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
     ++c->launches;
 
     // heaviest-first order of the target leaves
-    PH_CUDA_BUILD(cudaMalloc(&c->d_order, sizeof(int) * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&d_okeys, sizeof(unsigned) * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&d_okeys2, sizeof(unsigned) * n_leaves));
-    PH_CUDA_BUILD(cudaMalloc(&d_ovals, sizeof(int) * n_leaves));
+    unsigned *d_okeys = nullptr, *d_okeys2 = nullptr;
+    int* d_ovals = nullptr;
+    PH_WS(c->d_order, int, WS_ORDER, n_leaves);
+    PH_WS(d_okeys, unsigned, WS_ORDER_KEYS, n_leaves);
+    PH_WS(d_okeys2, unsigned, WS_ORDER_KEYS2, n_leaves);
+    PH_WS(d_ovals, int, WS_ORDER_VALS, n_leaves);
     order_keys_kernel<<<blocks_for(n_leaves, tb), tb, 0, st>>>(n_leaves, d_work, d_okeys, d_ovals);
     ++c->launches;
     {
         size_t sort_bytes = 0;
         PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairsDescending(nullptr, sort_bytes, d_okeys, d_okeys2, d_ovals, c->d_order, (int)n_leaves, 0, 32, st));
-        if (sort_bytes > tmp_bytes) {
-            cudaFree(d_tmp); d_tmp = nullptr;
-            PH_CUDA_BUILD(cudaMalloc(&d_tmp, sort_bytes));
-            tmp_bytes = sort_bytes;
-        }
-        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairsDescending(d_tmp, sort_bytes, d_okeys, d_okeys2, d_ovals, c->d_order, (int)n_leaves, 0, 32, st));
+        void* tmp = workspace(c, WS_CUB_TMP, sort_bytes);
+        if (!tmp) return PHOTONS_ENOMEM;
+        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairsDescending(tmp, sort_bytes, d_okeys, d_okeys2, d_ovals, c->d_order, (int)n_leaves, 0, 32, st));
     }
+    unsigned h_last = 0;
     PH_CUDA_BUILD(cudaMemcpyAsync(&h_last, d_okeys2, sizeof(unsigned), cudaMemcpyDeviceToHost, st));   // largest work
     PH_CUDA_BUILD(cudaStreamSynchronize(st));
     PH_CUDA_BUILD(cudaGetLastError());
@@ -423,12 +523,8 @@ int build_leaves_impl(Ctx* c)
     c->stats.n_chunks = h_nchunks;
     c->stats.n_leaf_pairs = (long long)h_tot[0];
     c->stats.pairs_evaluated = (long long)h_tot[1];
-    c->stats.max_leaves_per_target = (long long)(unsigned)h_last / M;
-
-done:
-    cudaFree(d_idx2); cudaFree(d_keys); cudaFree(d_keys2); cudaFree(d_blo); cudaFree(d_bhi); cudaFree(d_tmp);
-    cudaFree(d_nch); cudaFree(d_work); cudaFree(d_tot); cudaFree(d_okeys); cudaFree(d_okeys2); cudaFree(d_ovals);
-    return rc;
+    c->stats.max_leaves_per_target = (long long)h_last / M;
+    return PHOTONS_OK;
 }
 
 }  // namespace photons

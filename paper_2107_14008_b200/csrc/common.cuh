@@ -27,6 +27,17 @@ struct GTable {                 // Eq. 2 table
 
 constexpr int POLY_MAX_DEG = 20;
 
+// Grow-only device workspace: one buffer per role, allocated on first use and kept until photons_destroy, so
+// that repeated set_particles / build_leaves / short_range_acc steps do no cudaMalloc / cudaFree at all.
+enum WsSlot {
+    WS_POS, WS_MASS, WS_IN_POS, WS_IN_MASS, WS_FLAG, WS_OUT,
+    WS_PERM, WS_ORB_P0, WS_ORB_P1, WS_ORB_KEYS, WS_ORB_KEYS2, WS_ORB_VALS, WS_ORB_VALS2, WS_ORB_LO, WS_ORB_HI, WS_CUB_TMP,
+    WS_LEAF_CNT, WS_NODE_LO, WS_NODE_HI, WS_LEAF_CTR, WS_SLOT_SRC, WS_P64, WS_P32,
+    WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
+    WS_COUNT
+};
+struct DevBuf { void* p = nullptr; size_t cap = 0; };
+
 struct Ctx {
     photons_params p{};
     double r_s = 0, r_cut = 0;
@@ -49,8 +60,6 @@ struct Ctx {
     uint32_t* d_perm = nullptr;     // sorted position -> caller index
     int* d_slot_src = nullptr;      // slot -> caller index, -1 for padding slots
     int* d_leaf_cnt = nullptr;      // real particles per leaf
-    double* d_leaf_lo = nullptr;    // n_leaves x 3 tight bbox
-    double* d_leaf_hi = nullptr;
     double* d_leaf_ctr = nullptr;   // n_leaves x 3 (mixed: origin of the fp32 offsets)
     double* d_node_lo = nullptr;    // (2 n_leaves - 1) x 3, heap order
     double* d_node_hi = nullptr;
@@ -66,9 +75,16 @@ struct Ctx {
     float poly_c[POLY_MAX_DEG + 1]{};   // Q(s)/(2 r_s)^3 as a polynomial in t = 2 s/s_max - 1, Horner order
     double poly_err = 0;                // max |g_poly - g| over [0, x_cut] in exact arithmetic
 
+    DevBuf ws[WS_COUNT];
+
     photons_stats stats{};
     std::string err;
 };
+
+// pointer to at least `bytes` of device memory in slot `slot` (contents undefined after growth); nullptr and
+// c->err set if the allocation fails
+void* workspace(Ctx* c, int slot, size_t bytes);
+void workspace_free(Ctx* c);
 
 int fail(Ctx* c, int code, const char* fmt, ...);
 #define PH_CUDA(c, call)                                                                         \
