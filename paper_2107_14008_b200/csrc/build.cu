@@ -49,11 +49,13 @@ __global__ void fill_int_kernel(long long n, int* p, int v)
 }
 
 // P_out[q] = P_in[src[q]] (src == nullptr: identity), and the bounding boxes of the level-`level` nodes as
-// fp32 bit patterns (positions are >= 0, so the integer order of the bits is the float order)
-__global__ void orb_gather_bbox_kernel(long long n, int level, const uint32_t* __restrict__ src,
-                                       const float4* __restrict__ P_in, float4* __restrict__ P_out,
-                                       int* __restrict__ lo, int* __restrict__ hi)
+// fp32 bit patterns (positions are >= 0, so the integer order of the bits is the float order).  Reduced per
+// warp and, when the whole block sits in one node (the upper levels), per block, before the global atomics.
+__global__ void __launch_bounds__(256) orb_gather_bbox_kernel(long long n, int level, const uint32_t* __restrict__ src,
+                                                              const float4* __restrict__ P_in, float4* __restrict__ P_out,
+                                                              int* __restrict__ lo, int* __restrict__ hi)
 {
+    __shared__ int s_lo[8][3], s_hi[8][3];
     long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     const bool live = q < n;
     const long long qq = live ? q : n - 1;
@@ -61,16 +63,32 @@ __global__ void orb_gather_bbox_kernel(long long n, int level, const uint32_t* _
     if (live && P_out) P_out[q] = p;
     if (!lo) return;
     const long long seg = seg_of(n, level, qq);
+    const long long q_first = blockIdx.x * (long long)blockDim.x;
+    const long long q_last = min(q_first + blockDim.x, n) - 1;
+    const bool block_uniform = seg_of(n, level, q_first) == seg_of(n, level, q_last);
     const int v[3] = {__float_as_int(p.x), __float_as_int(p.y), __float_as_int(p.z)};
-    // warp-aggregate when the whole warp sits in one node
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long seg0 = __shfl_sync(0xffffffffu, seg, 0);
-    if (__all_sync(0xffffffffu, seg == seg0)) {
+    const bool warp_uniform = __all_sync(0xffffffffu, seg == seg0);
+    if (warp_uniform) {
         for (int a = 0; a < 3; ++a) {
             const int mn = __reduce_min_sync(0xffffffffu, v[a]), mx = __reduce_max_sync(0xffffffffu, v[a]);
-            if ((threadIdx.x & 31) == 0) { atomicMin(&lo[3 * seg + a], mn); atomicMax(&hi[3 * seg + a], mx); }
+            if (lane == 0) {
+                if (block_uniform) { s_lo[warp][a] = mn; s_hi[warp][a] = mx; }
+                else { atomicMin(&lo[3 * seg + a], mn); atomicMax(&hi[3 * seg + a], mx); }
+            }
         }
     } else if (live) {
         for (int a = 0; a < 3; ++a) { atomicMin(&lo[3 * seg + a], v[a]); atomicMax(&hi[3 * seg + a], v[a]); }
+    }
+    if (block_uniform) {     // then every warp is uniform too
+        __syncthreads();
+        if (threadIdx.x < 3) {
+            int mn = s_lo[0][threadIdx.x], mx = s_hi[0][threadIdx.x];
+            for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { mn = min(mn, s_lo[w][threadIdx.x]); mx = max(mx, s_hi[w][threadIdx.x]); }
+            atomicMin(&lo[3 * seg + threadIdx.x], mn);
+            atomicMax(&hi[3 * seg + threadIdx.x], mx);
+        }
     }
 }
 
@@ -104,13 +122,12 @@ __device__ __forceinline__ void cta_bitonic_sort(unsigned long long* key, int n2
 {
     for (int k = 2; k <= n2; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = threadIdx.x; i < n2; i += blockDim.x) {
-                const int l = i ^ j;
-                if (l > i) {
-                    const unsigned long long a = key[i], b = key[l];
-                    const bool up = (i & k) == 0;
-                    if ((a > b) == up) { key[i] = b; key[l] = a; }
-                }
+            for (int t = threadIdx.x; t < (n2 >> 1); t += blockDim.x) {
+                const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // the lower index of the t-th pair
+                const int l = i | j;
+                const unsigned long long a = key[i], b = key[l];
+                const bool up = (i & k) == 0;
+                if ((a > b) == up) { key[i] = b; key[l] = a; }
             }
             __syncthreads();
         }
@@ -138,12 +155,21 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
         const int nsub = 1 << sl;
         for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { blo[i] = 0x7fffffff; bhi[i] = 0; }
         __syncthreads();
-        for (int e = threadIdx.x; e < size; e += blockDim.x) {
-            const int sub = (int)seg_of(size, sl, e);
-            const float4 p = cur[e];
-            atomicMin(&blo[3 * sub], __float_as_int(p.x)); atomicMax(&bhi[3 * sub], __float_as_int(p.x));
-            atomicMin(&blo[3 * sub + 1], __float_as_int(p.y)); atomicMax(&bhi[3 * sub + 1], __float_as_int(p.y));
-            atomicMin(&blo[3 * sub + 2], __float_as_int(p.z)); atomicMax(&bhi[3 * sub + 2], __float_as_int(p.z));
+        for (int e0 = 0; e0 < size; e0 += blockDim.x) {       // whole warps enter: the votes below need all lanes
+            const int e = e0 + threadIdx.x;
+            const bool live = e < size;
+            const int sub = (int)seg_of(size, sl, live ? e : size - 1);
+            const float4 p = cur[live ? e : size - 1];
+            const int v[3] = {__float_as_int(p.x), __float_as_int(p.y), __float_as_int(p.z)};
+            const int sub0 = __shfl_sync(0xffffffffu, sub, 0);
+            if (__all_sync(0xffffffffu, sub == sub0)) {
+                for (int a = 0; a < 3; ++a) {
+                    const int mn = __reduce_min_sync(0xffffffffu, v[a]), mx = __reduce_max_sync(0xffffffffu, v[a]);
+                    if ((threadIdx.x & 31) == 0) { atomicMin(&blo[3 * sub + a], mn); atomicMax(&bhi[3 * sub + a], mx); }
+                }
+            } else if (live) {
+                for (int a = 0; a < 3; ++a) { atomicMin(&blo[3 * sub + a], v[a]); atomicMax(&bhi[3 * sub + a], v[a]); }
+            }
         }
         __syncthreads();
         for (int e = threadIdx.x; e < n2; e += blockDim.x) {
@@ -251,6 +277,8 @@ __global__ void node_bbox_kernel(int level, double* __restrict__ lo, double* __r
 // merged into runs of contiguous leaves with the same image shift, at most chunk_max slots long.
 // Pass 1 (chunks == nullptr) counts, pass 2 writes.
 
+constexpr int LIST_STASH = 128;   // list entries per leaf kept from the counting pass
+
 struct ListArgs {
     long long n_leaves;
     int depth, maxleaf, chunk_max;
@@ -259,6 +287,8 @@ struct ListArgs {
     const int* leaf_cnt;
     const long long* chunk_ptr;   // pass 2
     uint2* chunks;                // pass 2
+    uint2* stash;                 // pass 1: the first stash_cap entries of every leaf, stride stash_cap
+    int stash_cap;
     long long* n_chunks_of;       // pass 1: per leaf
     unsigned long long* totals;   // pass 1: [0] leaf pairs, [1] pairs evaluated
     long long* work_of;           // pass 1: slots in the list of each leaf (for the heaviest-first order)
@@ -279,7 +309,11 @@ __global__ void list_kernel(ListArgs a)
     stack[sp++] = 0;
     long long run_first = -1, run_n = 0, n_chunks = 0, n_pairs = 0, n_eval = 0, work = 0;
     int run_code = -1;
+    // Pass 1 counts and keeps the first stash_cap entries of every leaf; pass 2 (only the leaves whose list
+    // did not fit, the rest is a plain copy by list_copy_kernel) walks again and writes in place.
+    if (a.chunks && a.n_chunks_of[i] <= a.stash_cap) return;
     uint2* out = a.chunks ? a.chunks + a.chunk_ptr[i] : nullptr;
+    uint2* stash = a.chunks ? nullptr : a.stash + i * a.stash_cap;
     const int max_leaves_per_chunk = a.chunk_max / a.maxleaf;
 
     while (sp) {
@@ -315,14 +349,18 @@ __global__ void list_kernel(ListArgs a)
             ++run_n;
         } else {
             if (run_n > 0) {
-                if (out) out[n_chunks] = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+                const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+                if (out) out[n_chunks] = ent;
+                else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
                 ++n_chunks;
             }
             run_first = j; run_n = 1; run_code = code;
         }
     }
     if (run_n > 0) {
-        if (out) out[n_chunks] = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+        const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+        if (out) out[n_chunks] = ent;
+        else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
         ++n_chunks;
     }
     if (!a.chunks) {
@@ -331,6 +369,18 @@ __global__ void list_kernel(ListArgs a)
         atomicAdd(&a.totals[0], (unsigned long long)n_pairs);
         atomicAdd(&a.totals[1], (unsigned long long)n_eval);
     }
+}
+
+// one warp per leaf: stash -> CSR for the lists that fitted into the stash
+__global__ void list_copy_kernel(long long n_leaves, int stash_cap, const long long* __restrict__ chunk_ptr,
+                                 const uint2* __restrict__ stash, uint2* __restrict__ chunks)
+{
+    const long long i = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    if (i >= n_leaves) return;
+    const long long c0 = chunk_ptr[i];
+    const int cnt = (int)(chunk_ptr[i + 1] - c0);
+    if (cnt > stash_cap) return;
+    for (int k = threadIdx.x & 31; k < cnt; k += 32) chunks[c0 + k] = stash[i * stash_cap + k];
 }
 
 __global__ void order_keys_kernel(long long n_leaves, const long long* __restrict__ work, unsigned* __restrict__ keys, int* __restrict__ vals)
@@ -478,6 +528,8 @@ int build_leaves_impl(Ctx* c)
     la.L = c->p.boxsize; la.rcut = c->r_cut;
     la.node_lo = c->d_node_lo; la.node_hi = c->d_node_hi; la.leaf_cnt = c->d_leaf_cnt;
     la.chunk_ptr = nullptr; la.chunks = nullptr; la.n_chunks_of = d_nch; la.totals = d_tot; la.work_of = d_work;
+    la.stash_cap = LIST_STASH;
+    PH_WS(la.stash, uint2, WS_LIST_STASH, n_leaves * LIST_STASH);
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
     ++c->launches;
     {
@@ -494,8 +546,9 @@ int build_leaves_impl(Ctx* c)
     PH_CUDA_BUILD(cudaStreamSynchronize(st));
     PH_WS(c->d_chunks, uint2, WS_CHUNKS, std::max<long long>(h_nchunks, 1));
     la.chunk_ptr = c->d_chunk_ptr; la.chunks = c->d_chunks;
+    list_copy_kernel<<<blocks_for(32 * n_leaves, tb), tb, 0, st>>>(n_leaves, LIST_STASH, c->d_chunk_ptr, la.stash, c->d_chunks);
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
-    ++c->launches;
+    c->launches += 2;
 
     // heaviest-first order of the target leaves
     unsigned *d_okeys = nullptr, *d_okeys2 = nullptr;
