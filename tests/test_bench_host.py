@@ -1,0 +1,109 @@
+"""Host-side logic of bench.py that needs no GPU: the multi-rank aggregation (world size 2 over gloo), the
+replica seeding, the flop convention, and the polynomial behind PHOTONS_G_POLY against the oracle's g."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        # rank r took (10 + 5 r) ms for (1000 + r) units
+        ms, units = bench.aggregate(10.0 + 5.0 * rank, 1000.0 + rank, dist)
+        q.put((rank, ms, units))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_aggregate_is_max_time_sum_units_gloo_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, units in out:
+        assert ms == 15.0            # MAX over ranks
+        assert units == 2001.0       # SUM over ranks
+
+
+def test_aggregate_single_process_is_identity():
+    import bench
+    assert bench.aggregate(3.5, 7.0, None) == (3.5, 7.0)
+
+
+def test_replicas_have_their_own_seed():
+    import bench
+    from paper_2107_14008_b200 import workloads
+    cfg = workloads.CONFIGS[4]
+    assert bench.rank_config(cfg, 0) is cfg
+    seeds = {bench.rank_config(cfg, r).seed for r in range(8)}
+    assert len(seeds) == 8
+    assert all(bench.rank_config(cfg, r).n == cfg.n for r in range(8))
+
+
+def test_flop_convention_matches_design():
+    import bench
+    assert bench.flops_per_pair("poly", 12) == 46.0      # (8+12) FFMA x 2 + 3 FADD + 2 FMUL + 1 MUFU
+    assert bench.flops_per_pair("poly", 13) == 48.0
+    assert bench.PAPER_FLOPS_PER_PAIR == 51.0
+    # peak = SMs x lanes x 2 x clock
+    assert bench.SM_COUNT * bench.FP32_LANES_PER_SM * 2 * 1.965e9 == pytest.approx(74.45e12, rel=1e-4)
+
+
+def test_headline_params_follow_the_config():
+    import bench
+    from paper_2107_14008_b200 import workloads
+    p = bench.headline_params(workloads.CONFIGS[4])
+    assert (p["n_pm"], p["maxleaf"], p["precision"], p["g_mode"]) == (256, 32, "fp32", "poly")
+    assert p["close_pair_radius"] == 0.0
+    p1 = bench.headline_params(workloads.CONFIGS[1])
+    assert p1["close_pair_radius"] == pytest.approx(0.02 * 6 * 1.2 / 32)
+
+
+@pytest.mark.parametrize("degree,bound", [(10, 3e-6), (11, 5e-7), (12, 8e-8), (13, 1.2e-8), (14, 2e-9)])
+def test_poly_g_against_oracle_T(oracle, degree, bound):
+    """The FMA-pipe polynomial (host-only hook of the library) reproduces Eq. 1 as the oracle evaluates it:
+    g(r) = 1 - s^(3/2) Q(t), s = (r/2r_s)^2, t = 2 s/9 - 1."""
+    from paper_2107_14008_b200 import build, binding
+    build.build()
+    coeffs, err = binding.poly_fit(degree, 6.0)
+    x = np.linspace(0.0, 3.0, 6001)
+    s = x * x
+    t = 2.0 * s / 9.0 - 1.0
+    g = 1.0 - s ** 1.5 * np.polyval(coeffs[::-1], t)
+    dev = np.abs(g - oracle.oracle_T(x)).max()
+    assert dev <= bound
+    assert err == pytest.approx(dev, rel=0.05, abs=1e-12)     # the library's own error estimate is honest
+    # Newtonian limit and the value at the cut
+    assert g[0] == 1.0
+    assert g[-1] == pytest.approx(4.39849652838829e-4, abs=bound)
+
+
+def test_poly_fit_rejects_bad_arguments():
+    from paper_2107_14008_b200 import build, binding
+    build.build()
+    for deg, rc in ((0, 6.0), (21, 6.0), (12, 0.0), (12, 6.5)):
+        with pytest.raises(binding.PhotonsError):
+            binding.poly_fit(deg, rc)
