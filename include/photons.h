@@ -85,6 +85,9 @@ typedef struct {
                                  0 = default (128); multiple of maxleaf, <= 256 */
     int warps_per_leaf;       /* warps of the CTA that owns one target leaf; they split its source list.
                                  0 = default; 1, 2, 4 or 8 */
+    int targets_per_lane;     /* fp32/mixed kernels: targets a lane keeps in registers, 1, 2 or 4 (the warp then splits
+                                 into 32 T / maxleaf groups that take alternate source pairs); 0 = default.
+                                 Available: maxleaf 16: 1, 2; 32: 1, 2, 4; 64: 2, 4; 128: 4 */
     int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12) */
 } photons_params;
 
@@ -153,7 +156,8 @@ int photons_get_stats(photons_ctx* ctx, photons_stats* stats);
  * 4 = FFMA2 with 2 MUFU.RSQ per 8 (FFMA2 lanes counted), 5 = LDS.128 broadcast, 6 = FFMA with immediates,
  * 7 = FFMA2 with 4 ALU-pipe ops per 8 (FFMA2 lanes counted), 8 = FADD2, 9 = FMUL2, 10 = FFMA2 without
  * operand reuse; 11..15 = the pair core's mix per step, 24 FFMA2 in two dependent chains (14) plus 2 MUFU.RSQ (11),
- * plus 2 FSETP+FSEL (12), or plus 2 broadcast LDS.128 (13), or plus both (15) — FFMA2 lanes counted.
+ * plus 2 FSETP+FSEL (12), or plus 2 broadcast LDS.128 (13), or plus both (15); 16 / 17 = kind 10 plus 4 / 8 integer
+ * ALU ops per 8 FFMA2 — FFMA2 lanes counted.
  * kind + 100 b (b = 1..7) runs the probe with only b resident blocks of 8 warps per SM.  *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction
  * counts 2 per lane; multiply FMA rates by 2 for flops).  Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
 int photons_peak_probe(int device, int kind, double* out);

@@ -115,6 +115,7 @@ void photons_default_params(photons_params* p)
     p->close_pair_radius = 0.0;
     p->chunk_max = 0;
     p->warps_per_leaf = 0;
+    p->targets_per_lane = 0;
     p->poly_degree = 0;
 }
 
@@ -152,6 +153,13 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.warps_per_leaf == 0) p.warps_per_leaf = 4;
     if (p.warps_per_leaf != 1 && p.warps_per_leaf != 2 && p.warps_per_leaf != 4 && p.warps_per_leaf != 8)
         return create_fail(err_buf, err_len, PHOTONS_EINVAL, "warps_per_leaf must be 1, 2, 4 or 8");
+    if (p.targets_per_lane == 0) p.targets_per_lane = p.maxleaf <= 32 ? 1 : p.maxleaf / 32;
+    {
+        const int t = p.targets_per_lane, m = p.maxleaf;
+        const bool ok = (m == 16 && (t == 1 || t == 2)) || (m == 32 && (t == 1 || t == 2 || t == 4)) ||
+                        (m == 64 && (t == 2 || t == 4)) || (m == 128 && t == 4);
+        if (!ok) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "targets_per_lane not available for this maxleaf");
+    }
     if (p.poly_degree == 0) p.poly_degree = 12;
     if (p.poly_degree < 10 || p.poly_degree > 14) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "poly_degree must be 10..14");
 

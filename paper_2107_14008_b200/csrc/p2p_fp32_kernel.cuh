@@ -2,7 +2,8 @@
 //
 // Mapping:
 //   CTA            one target leaf (Alg. 1 L96); its W warps split the leaf's source list
-//   lane           T = maxleaf/32 targets in registers (maxleaf 16: the two half-warps take the same 16
+//   lane           T targets in registers; the warp is split into 32 T / maxleaf lane groups that take
+//                  alternate source pairs (maxleaf 16: the two half-warps take the same 16
 //                  targets and alternate source pairs)
 //   source staging runs of contiguous source leaves, one TMA bulk copy each into a per-warp mbarrier ring
 //   pair core      two sources per lane per step in packed fp32 (add/mul/fma.rn.f32x2 -> FADD2/FMUL2/FFMA2),
@@ -12,6 +13,13 @@
 #pragma once
 #include "common.cuh"
 #include "pipeline.cuh"
+
+#ifndef PHOTONS_UNROLL_T1
+#define PHOTONS_UNROLL_T1 4   // source pairs per loop iteration with one target per lane (measured: 4 beats 2 by 3 %)
+#endif
+#ifndef PHOTONS_UNROLL_T2
+#define PHOTONS_UNROLL_T2 2   // ... with two targets per lane
+#endif
 
 namespace photons {
 
@@ -132,29 +140,35 @@ __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, f
 // The same for NCH independent chains (targets x unrolled source pairs) at once.  The polynomial is a chain
 // of dependent FFMA2s, one every ~4 clocks per warp; writing the Horner steps of all chains side by side
 // keeps NCH of them in flight, which is what lets a few warps per scheduler saturate the FMA pipe.
+// kc: the loop constants (polynomial coefficients, tk, r_cut^2) as one local object
+struct LoopConst {
+    float pc[POLY_MAX_DEG + 1];
+    float tk, rcut2;
+};
+
 template <int GKIND, int GPAR, int NCH>
-__device__ __forceinline__ void weights(const P32Args& a, const float2* tab, const float2 (&r2)[NCH], const float2 (&gm)[NCH],
-                                        float2 (&w)[NCH])
+__device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, const float2* tab, const float2 (&r2)[NCH],
+                                        const float2 (&gm)[NCH], float2 (&w)[NCH])
 {
     if (GKIND == GM_POLY) {
         float2 idr[NCH], t[NCH], q[NCH];
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
             idr[c] = f2(rsq(r2[c].x), rsq(r2[c].y));
-            t[c] = __ffma2_rn(r2[c], dup(a.tk), dup(-1.0f));
-            q[c] = __ffma2_rn(dup(a.pc[0]), t[c], dup(a.pc[1]));
+            t[c] = __ffma2_rn(r2[c], dup(kc.tk), dup(-1.0f));
+            q[c] = __ffma2_rn(dup(kc.pc[0]), t[c], dup(kc.pc[1]));
         }
 #pragma unroll
         for (int k = 2; k <= GPAR; ++k) {
 #pragma unroll
-            for (int c = 0; c < NCH; ++c) q[c] = __ffma2_rn(q[c], t[c], dup(a.pc[k]));
+            for (int c = 0; c < NCH; ++c) q[c] = __ffma2_rn(q[c], t[c], dup(kc.pc[k]));
         }
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
             const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
             const float2 u = __ffma2_rn(idr2, idr[c], f2(-q[c].x, -q[c].y));
             const float2 v = __fmul2_rn(u, gm[c]);
-            w[c] = f2(r2[c].x < a.rcut2 ? v.x : 0.f, r2[c].y < a.rcut2 ? v.y : 0.f);
+            w[c] = f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f);
         }
     } else {
 #pragma unroll
@@ -178,7 +192,7 @@ static __device__ __noinline__ double close_pair_weight(double r2, double gm, do
 
 // ---------------------------------------------------------------------------------------------------------
 
-template <int T, bool HALF, int GKIND, int GPAR, bool CLOSE>
+template <int T, int HS, int GKIND, int GPAR, bool CLOSE>
 __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -193,13 +207,24 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 
     const long long leaf = a.order[a.first + blockIdx.x];
     const long long slot0 = leaf * M;
-    const int half = HALF ? lane >> 4 : 0;
-    const int pstep = HALF ? 2 : 1;
+    // HS groups of LG = 32/HS lanes: a lane owns T targets (lane-in-group + LG t), the groups take alternate
+    // source pairs.  MAXLEAF = T * LG.  More targets per lane = fewer shared-memory reads per pair.
+    constexpr int LG = 32 / HS;
+    const int half = HS > 1 ? lane / LG : 0;
+    const int pstep = HS;
 
     if (GKIND == GM_TABLE) {   // the interpolation table lives in shared memory (Fig. 1)
         for (int i = threadIdx.x; i <= a.tn; i += blockDim.x) tab[i] = a.table[i];
         __syncthreads();
     }
+
+    LoopConst kc;
+    if (GKIND == GM_POLY) {
+#pragma unroll
+        for (int k = 0; k <= GPAR; ++k) kc.pc[k] = a.pc[k];
+    }
+    kc.tk = a.tk;
+    kc.rcut2 = a.rcut2;
 
     // targets -> registers (Alg. 1 L99)
     float tx[T], ty[T], tz[T];
@@ -207,7 +232,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     int tslot[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        const int l = HALF ? (lane & 15) : lane + 32 * t;
+        const int l = (lane % LG) + LG * t;
         tslot[t] = (int)slot0 + l;
         const float* b = a.p32 + (size_t)(tslot[t] >> 1) * 8 + (tslot[t] & 1);
         tx[t] = b[0]; ty[t] = b[2]; tz[t] = b[4];
@@ -319,7 +344,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                 }
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
                 // U source pairs x T targets = NCH independent chains per iteration
-                constexpr int U = T == 1 ? 2 : 1;
+                constexpr int U = T == 1 ? PHOTONS_UNROLL_T1 : T == 2 ? PHOTONS_UNROLL_T2 : 1;
                 constexpr int NCH = U * T;
                 auto step = [&](const int p, const bool with_seam) {
                     float2 dx[NCH], dy[NCH], dz[NCH], r2[NCH], gm[NCH], w[NCH];
@@ -343,7 +368,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                             r2[c] = f2(fmaxf(r2[c].x, a.rclose2), fmaxf(r2[c].y, a.rclose2));
                         }
                     }
-                    weights<GKIND, GPAR, NCH>(a, tab, r2, gm, w);
+                    weights<GKIND, GPAR, NCH>(a, kc, tab, r2, gm, w);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
 #pragma unroll
@@ -400,12 +425,13 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         if (k + N_STAGES < n_my) issue(k + N_STAGES, batch);
     }
 
-    if (HALF) {
+#pragma unroll
+    for (int o = 16; o >= LG; o >>= 1) {     // add the groups' partial sums (fixed order)
 #pragma unroll
         for (int t = 0; t < T; ++t) {
-            ax[t] += __shfl_xor_sync(0xffffffffu, ax[t], 16);
-            ay[t] += __shfl_xor_sync(0xffffffffu, ay[t], 16);
-            az[t] += __shfl_xor_sync(0xffffffffu, az[t], 16);
+            ax[t] += __shfl_xor_sync(0xffffffffu, ax[t], o);
+            ay[t] += __shfl_xor_sync(0xffffffffu, ay[t], o);
+            az[t] += __shfl_xor_sync(0xffffffffu, az[t], o);
         }
     }
     // sum the warps' partial accelerations in a fixed order (deterministic), then scatter to caller order
@@ -426,7 +452,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     }
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        if (HALF && lane >= 16) continue;
+        if (lane >= LG) continue;
         const int dst = a.slot_src[tslot[t]];
         if (dst < 0) continue;
         if (a.out_f32) {
@@ -448,13 +474,20 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
 {
     const int W = c->p.warps_per_leaf;
     const int M = c->p.maxleaf;
-    const int T = M <= 32 ? 1 : M / 32;
+    const int T = c->p.targets_per_lane;
     const size_t smem = p32_smem_bytes(c, T);
     void (*kern)(P32Args) = nullptr;
-    if (M == 16) kern = p2p_fp32_kernel<1, true, GKIND, GPAR, CLOSE>;
-    else if (M == 32) kern = p2p_fp32_kernel<1, false, GKIND, GPAR, CLOSE>;
-    else if (M == 64) kern = p2p_fp32_kernel<2, false, GKIND, GPAR, CLOSE>;
-    else kern = p2p_fp32_kernel<4, false, GKIND, GPAR, CLOSE>;
+    switch (M * 8 + T) {   // (MAXLEAF, targets per lane) -> (T, lane groups)
+        case 16 * 8 + 1: kern = p2p_fp32_kernel<1, 2, GKIND, GPAR, CLOSE>; break;
+        case 16 * 8 + 2: kern = p2p_fp32_kernel<2, 4, GKIND, GPAR, CLOSE>; break;
+        case 32 * 8 + 1: kern = p2p_fp32_kernel<1, 1, GKIND, GPAR, CLOSE>; break;
+        case 32 * 8 + 2: kern = p2p_fp32_kernel<2, 2, GKIND, GPAR, CLOSE>; break;
+        case 32 * 8 + 4: kern = p2p_fp32_kernel<4, 4, GKIND, GPAR, CLOSE>; break;
+        case 64 * 8 + 2: kern = p2p_fp32_kernel<2, 1, GKIND, GPAR, CLOSE>; break;
+        case 64 * 8 + 4: kern = p2p_fp32_kernel<4, 2, GKIND, GPAR, CLOSE>; break;
+        case 128 * 8 + 4: kern = p2p_fp32_kernel<4, 1, GKIND, GPAR, CLOSE>; break;
+        default: return fail(c, PHOTONS_EINVAL, "targets_per_lane %d is not available for maxleaf %d", T, M);
+    }
     PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
     ++c->launches;

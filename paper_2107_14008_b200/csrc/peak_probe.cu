@@ -67,6 +67,11 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, float a_in, floa
         } else if (KIND == 10) {    // FFMA2 with both multiplicands distinct per chain (no operand reuse)
 #pragma unroll
             for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
+        } else if (KIND == 16 || KIND == 17) {   // 8 FFMA2 without operand reuse : 4 (16) or 8 (17) ALU-pipe ops
+#pragma unroll
+            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
+#pragma unroll
+            for (int i = 0; i < (KIND == 16 ? 4 : 8); ++i) x[i] = __int_as_float(__float_as_int(x[i]) ^ (it + i));
         } else if (KIND >= 11 && KIND <= 15) {
             // the pair core's instruction mix per step (two pairs per lane): 24 FFMA2-class in two dependent
             // chains (Horner), plus 11: 2 MUFU.RSQ (single instruction, ftz)   12: + 2 x (FSETP + FSEL)
@@ -132,7 +137,7 @@ extern "C" int photons_peak_probe(int device, int kind, double* out)
     // kind + 100 * b: the same probe with only b (1..7) resident blocks of 8 warps per SM (occupancy sweep)
     g_blocks_per_sm = 8;
     if (kind >= 100) { g_blocks_per_sm = kind / 100; kind %= 100; }
-    if (!out || kind < 0 || kind > 15 || g_blocks_per_sm < 1 || g_blocks_per_sm > 8) return PHOTONS_EINVAL;
+    if (!out || kind < 0 || kind > 17 || g_blocks_per_sm < 1 || g_blocks_per_sm > 8) return PHOTONS_EINVAL;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) {
         cudaGetLastError();
@@ -159,7 +164,9 @@ extern "C" int photons_peak_probe(int device, int kind, double* out)
         case 12: e = run_probe<12>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
         case 13: e = run_probe<13>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
         case 14: e = run_probe<14>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
-        default: e = run_probe<15>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        case 15: e = run_probe<15>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
+        case 16: e = run_probe<16>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        default: e = run_probe<17>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
     }
     cudaFree(d_out);
     if (e != cudaSuccess) return PHOTONS_ECUDA;

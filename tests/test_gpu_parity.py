@@ -178,6 +178,20 @@ def test_launch_shape_invariance(B, c1):
         assert _err(out, ref) <= TOL_FP32
 
 
+@pytest.mark.parametrize("maxleaf,tpl", [(16, 1), (16, 2), (32, 1), (32, 2), (32, 4), (64, 2), (64, 4), (128, 4)])
+def test_lane_mappings(B, c1, maxleaf, tpl):
+    # every (MAXLEAF, targets per lane) shape of the fp32 kernel, with and without the exact close-pair path
+    cfg, pos, mass, ref, _ = c1
+    for prec, g, tol in (("fp32", "poly", TOL_FP32), ("mixed", "table", TOL_TABLE), ("fp32", "direct", TOL_FP32)):
+        out, _ = _run(B, cfg, pos, mass, precision=prec, g_mode=g, maxleaf=maxleaf, targets_per_lane=tpl,
+                      close_pair_radius=_close(cfg))
+        assert _err(out, ref) <= tol
+    out, _ = _run(B, cfg, pos, mass, precision="fp32", g_mode="poly", maxleaf=maxleaf, targets_per_lane=tpl)
+    assert _err(out, ref) <= 1e-4
+    with pytest.raises(B.PhotonsError):
+        B.Photons(maxleaf=128, targets_per_lane=1)
+
+
 def test_pairs_evaluated_and_list_cover(B, c1):
     """Host-visible feeder outputs: the permutation is a permutation, leaves are ORB-balanced, and the
     interaction list of every target leaf holds every leaf that has a particle pair inside r_cut (A11)."""
