@@ -87,7 +87,7 @@ typedef struct {
                                  0 = default; 1, 2, 4 or 8 */
     int targets_per_lane;     /* fp32/mixed kernels: targets a lane keeps in registers, 1, 2 or 4 (the warp then splits
                                  into 32 T / maxleaf groups that take alternate source pairs); 0 = default.
-                                 Available: maxleaf 16: 1, 2; 32: 1, 2, 4; 64: 2, 4; 128: 4 */
+                                 Available: maxleaf 16: 1, 2; 32: 1, 2; 64: 2; 128: 4 */
     int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12) */
 } photons_params;
 

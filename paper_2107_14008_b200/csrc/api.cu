@@ -156,8 +156,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.targets_per_lane == 0) p.targets_per_lane = p.maxleaf <= 32 ? 1 : p.maxleaf / 32;
     {
         const int t = p.targets_per_lane, m = p.maxleaf;
-        const bool ok = (m == 16 && (t == 1 || t == 2)) || (m == 32 && (t == 1 || t == 2 || t == 4)) ||
-                        (m == 64 && (t == 2 || t == 4)) || (m == 128 && t == 4);
+        const bool ok = (m == 16 && (t == 1 || t == 2)) || (m == 32 && (t == 1 || t == 2)) || (m == 64 && t == 2) || (m == 128 && t == 4);
         if (!ok) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "targets_per_lane not available for this maxleaf");
     }
     if (p.poly_degree == 0) p.poly_degree = 12;
@@ -364,7 +363,7 @@ int photons_get_interaction_list(photons_ctx* ctx, long long* chunk_ptr, int* fi
         for (size_t i = 0; i < h.size(); ++i) {
             if (first_leaf) first_leaf[i] = (int)(h[i].x / (unsigned)c->p.maxleaf);
             if (n_leaf) n_leaf[i] = (int)((h[i].y & 0xffffu) / (unsigned)c->p.maxleaf);
-            if (shift_code) shift_code[i] = (int)((h[i].y >> 16) & 31u);
+            if (shift_code) shift_code[i] = entry_shift_code(h[i].y);
         }
     }
     return PHOTONS_OK;

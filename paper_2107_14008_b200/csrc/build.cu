@@ -319,7 +319,7 @@ __global__ void list_kernel(ListArgs a)
     while (sp) {
         const long long node = stack[--sp];
         double g2 = 0;
-        int code = 0, mul = 1;
+        int code = 0, shl = 16;       // the three shift fields of entry_pack, without the slot count
         bool ambiguous = false;
         for (int x = 0; x < 3; ++x) {
             const double nl = a.node_lo[3 * node + x], nh = a.node_hi[3 * node + x];
@@ -329,8 +329,8 @@ __global__ void list_kernel(ListArgs a)
             dc -= a.L * img;
             const double gap = fmax(0.0, fabs(dc) - hw);
             g2 += gap * gap;
-            code += mul * (1 - (int)img);
-            mul *= 3;
+            code |= (1 - (int)img) << shl;
+            shl += 2;
             // the image is unique for every pair inside r_cut iff 2 r_cut + extents < L (A10)
             if (2.0 * a.rcut + 2.0 * hw >= a.L) ambiguous = true;
         }
@@ -341,7 +341,7 @@ __global__ void list_kernel(ListArgs a)
             continue;
         }
         const long long j = node - leaf0;
-        if (ambiguous) code = SHIFT_PER_PAIR;
+        if (ambiguous) code = (int)entry_pack(0, 0, 0, 0, true);
         ++n_pairs;
         n_eval += (long long)my_cnt * a.leaf_cnt[j];
         work += a.maxleaf;
@@ -349,7 +349,7 @@ __global__ void list_kernel(ListArgs a)
             ++run_n;
         } else {
             if (run_n > 0) {
-                const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+                const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
                 if (out) out[n_chunks] = ent;
                 else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
                 ++n_chunks;
@@ -358,7 +358,7 @@ __global__ void list_kernel(ListArgs a)
         }
     }
     if (run_n > 0) {
-        const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | ((unsigned)run_code << 16));
+        const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
         if (out) out[n_chunks] = ent;
         else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
         ++n_chunks;

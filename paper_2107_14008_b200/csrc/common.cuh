@@ -12,10 +12,21 @@ namespace photons {
 
 // Interaction-list entry ("chunk"): a run of contiguous source leaves staged as one bulk copy.
 //   .x = first particle slot of the run (leaf * maxleaf)
-//   .y = bits 0..15 number of slots in the run, bits 16..20 shift code 0..26
-//        ((sx+1) + 3 (sy+1) + 9 (sz+1), s = box lengths added to the source) or 27 = per-pair minimum image
-constexpr int SHIFT_NONE = 13;      // code of (0,0,0)
-constexpr int SHIFT_PER_PAIR = 27;  // degenerate geometry: take the minimum image per pair (A10)
+//   .y = bits 0..15 number of slots in the run; bits 16-17, 18-19, 20-21 = sx + 1, sy + 1, sz + 1 with
+//        s in {-1, 0, +1} the box lengths added to the source; bit 22 = take the minimum image per pair
+//        instead (degenerate geometry, A10)
+constexpr unsigned ENTRY_PER_PAIR = 1u << 22;
+__host__ __device__ inline unsigned entry_pack(int slots, int sx, int sy, int sz, bool per_pair)
+{
+    return per_pair ? ((unsigned)slots | (1u << 16) | (1u << 18) | (1u << 20) | ENTRY_PER_PAIR)
+                    : ((unsigned)slots | ((unsigned)(sx + 1) << 16) | ((unsigned)(sy + 1) << 18) | ((unsigned)(sz + 1) << 20));
+}
+// the shift code of include/photons.h: (sx+1) + 3 (sy+1) + 9 (sz+1), or 27 = per pair
+__host__ __device__ inline int entry_shift_code(unsigned y)
+{
+    if (y & ENTRY_PER_PAIR) return 27;
+    return (int)((y >> 16) & 3u) + 3 * (int)((y >> 18) & 3u) + 9 * (int)((y >> 20) & 3u);
+}
 constexpr int N_STAGES = 3;         // shared-memory ring depth per warp
 
 struct GTable {                 // Eq. 2 table

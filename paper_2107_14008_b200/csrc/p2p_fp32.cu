@@ -17,7 +17,9 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
 {
     a.p32 = c->d_p32; a.p64 = c->d_p64; a.ctr = c->d_leaf_ctr; a.slot_src = c->d_slot_src;
     a.chunk_ptr = c->d_chunk_ptr; a.chunks = c->d_chunks; a.order = c->d_order; a.first = first;
-    a.maxleaf = c->p.maxleaf; a.chunk_max = c->p.chunk_max; a.mixed = c->p.precision == PHOTONS_MIXED;
+    a.maxleaf = c->p.maxleaf; a.log2m = 0;
+    while ((1 << a.log2m) < a.maxleaf) ++a.log2m;
+    a.chunk_max = c->p.chunk_max; a.mixed = c->p.precision == PHOTONS_MIXED;
     a.L = (float)c->p.boxsize; a.invL = (float)(1.0 / c->p.boxsize);
     a.rcut2 = (float)(c->r_cut * c->r_cut);
     a.rclose2 = (float)(c->p.close_pair_radius * c->p.close_pair_radius);

@@ -35,7 +35,7 @@ struct P32Args {
     const uint2* chunks;
     const int* order;
     long long first;
-    int maxleaf, chunk_max, mixed;
+    int maxleaf, log2m, chunk_max, mixed;
     float L, invL, rcut2, rclose2;
     double Ld, inv2rs_d, rclose_d, wclose_d;   // close pairs: g(r_close)/r_close^3 in fp64
     float inv2rs;              // 1 / 2 r_s
@@ -192,7 +192,7 @@ static __device__ __noinline__ double close_pair_weight(double r2, double gm, do
 
 // ---------------------------------------------------------------------------------------------------------
 
-template <int T, int HS, int GKIND, int GPAR, bool CLOSE>
+template <int T, int HS, bool MIXED, int GKIND, int GPAR, bool CLOSE>
 __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         ax[t] = ay[t] = az[t] = 0.0;
     }
     double cix = 0, ciy = 0, ciz = 0;
-    if (a.mixed) { cix = a.ctr[3 * leaf]; ciy = a.ctr[3 * leaf + 1]; ciz = a.ctr[3 * leaf + 2]; }
+    if (MIXED) { cix = a.ctr[3 * leaf]; ciy = a.ctr[3 * leaf + 1]; ciz = a.ctr[3 * leaf + 2]; }
 
     const long long c0 = a.chunk_ptr[leaf], c1 = a.chunk_ptr[leaf + 1];
     const long long n_all = c1 - c0;
@@ -262,30 +262,31 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         const uint2 v = (k >> 5) == cur_batch ? dcur : dnext;       // warp-uniform choice
         return make_uint2(__shfl_sync(0xffffffffu, v.x, k & 31), __shfl_sync(0xffffffffu, v.y, k & 31));
     };
-    auto issue = [&](int k, int cur_batch) {
+    // stage st of the ring: shared-memory addresses kept in registers, stage index and phase bit stepped by hand
+    const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
+    auto issue = [&](int k, int cur_batch, int st) {
         const uint2 e = entry(k, cur_batch);
         if (lane == 0) {
-            const int st = k % N_STAGES;
             const uint32_t bytes = (e.y & 0xffffu) * 16u;
-            mbar_expect_tx(&bars[st], bytes);
-            bulk_g2s(ring + (size_t)st * stage_bytes, a.p32 + (size_t)e.x * 4, bytes, &bars[st]);
+            mbar_expect_tx_u32(bars_u32 + 8u * st, bytes);
+            bulk_g2s_u32(ring_u32 + (uint32_t)(st * stage_bytes), a.p32 + (size_t)e.x * 4, bytes, bars_u32 + 8u * st);
         }
     };
-    for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k, 0);
+    for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k, 0, k);
 
+    int st = 0;
+    uint32_t phase = 0;
     for (int k = 0; k < n_my; ++k) {
-        const int st = k % N_STAGES;
         const int batch = k >> 5;
         if ((k & 31) == 0 && k > 0) { dcur = dnext; dnext = load_batch(batch + 1); }
         const uint2 e = entry(k, batch);
-        mbar_wait(&bars[st], (uint32_t)(k / N_STAGES) & 1u);
+        mbar_wait_u32(bars_u32 + 8u * st, phase);
         const int ns = (int)(e.y & 0xffffu);
-        const int code = (int)((e.y >> 16) & 31u);
         const float4* src = reinterpret_cast<const float4*>(ring + (size_t)st * stage_bytes);
-        const bool per_pair = code == SHIFT_PER_PAIR;
-        const int sxi = per_pair ? 0 : code % 3 - 1, syi = per_pair ? 0 : (code / 3) % 3 - 1, szi = per_pair ? 0 : code / 9 - 1;
+        const bool per_pair = (e.y & ENTRY_PER_PAIR) != 0;
+        const int sxi = (int)((e.y >> 16) & 3u) - 1, syi = (int)((e.y >> 18) & 3u) - 1, szi = (int)((e.y >> 20) & 3u) - 1;
         // MIXED: every source leaf of the run has its own origin; ABS: one block = the whole run
-        const int blk = a.mixed ? M : ns;
+        const int blk = MIXED ? M : ns;
 
         float px[T], py[T], pz[T];       // fp32 partial sums of this run (level 1 of the accumulation)
 #pragma unroll
@@ -296,8 +297,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             // targets as seen from this block: d = (r_j + sadd) - q
             float qx[T], qy[T], qz[T];
             float sax = 0.f, say = 0.f, saz = 0.f;
-            if (a.mixed) {
-                const long long jl = (long long)(e.x + b0) / M;
+            if (MIXED) {
+                const long long jl = (long long)((e.x + b0) >> a.log2m);
                 const float dcx = (float)((a.ctr[3 * jl] + a.Ld * sxi) - cix);
                 const float dcy = (float)((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy);
                 const float dcz = (float)((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz);
@@ -422,7 +423,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             }
         }
         __syncwarp();
-        if (k + N_STAGES < n_my) issue(k + N_STAGES, batch);
+        if (k + N_STAGES < n_my) issue(k + N_STAGES, batch, st);
+        if (++st == N_STAGES) { st = 0; phase ^= 1u; }
     }
 
 #pragma unroll
@@ -477,17 +479,18 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     const int T = c->p.targets_per_lane;
     const size_t smem = p32_smem_bytes(c, T);
     void (*kern)(P32Args) = nullptr;
+    const bool mixed = c->p.precision == PHOTONS_MIXED;
+#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR, CLOSE> : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR, CLOSE>)
     switch (M * 8 + T) {   // (MAXLEAF, targets per lane) -> (T, lane groups)
-        case 16 * 8 + 1: kern = p2p_fp32_kernel<1, 2, GKIND, GPAR, CLOSE>; break;
-        case 16 * 8 + 2: kern = p2p_fp32_kernel<2, 4, GKIND, GPAR, CLOSE>; break;
-        case 32 * 8 + 1: kern = p2p_fp32_kernel<1, 1, GKIND, GPAR, CLOSE>; break;
-        case 32 * 8 + 2: kern = p2p_fp32_kernel<2, 2, GKIND, GPAR, CLOSE>; break;
-        case 32 * 8 + 4: kern = p2p_fp32_kernel<4, 4, GKIND, GPAR, CLOSE>; break;
-        case 64 * 8 + 2: kern = p2p_fp32_kernel<2, 1, GKIND, GPAR, CLOSE>; break;
-        case 64 * 8 + 4: kern = p2p_fp32_kernel<4, 2, GKIND, GPAR, CLOSE>; break;
-        case 128 * 8 + 4: kern = p2p_fp32_kernel<4, 1, GKIND, GPAR, CLOSE>; break;
+        case 16 * 8 + 1: kern = PH_SHAPE(1, 2); break;
+        case 16 * 8 + 2: kern = PH_SHAPE(2, 4); break;
+        case 32 * 8 + 1: kern = PH_SHAPE(1, 1); break;
+        case 32 * 8 + 2: kern = PH_SHAPE(2, 2); break;
+        case 64 * 8 + 2: kern = PH_SHAPE(2, 1); break;
+        case 128 * 8 + 4: kern = PH_SHAPE(4, 1); break;
         default: return fail(c, PHOTONS_EINVAL, "targets_per_lane %d is not available for maxleaf %d", T, M);
     }
+#undef PH_SHAPE
     PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
     ++c->launches;
@@ -503,6 +506,8 @@ static int launch_p32_close(Ctx* c, const P32Args& a, long long count, cudaStrea
 }
 
 int launch_p32_poly(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
+template <int DEG>
+int launch_p32_poly_deg(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 int launch_p32_table(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 int launch_p32_direct(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 

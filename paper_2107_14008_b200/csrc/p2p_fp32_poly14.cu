@@ -1,0 +1,12 @@
+// Instantiations of the fp32 kernel with the degree-14 polynomial g (PHOTONS_G_POLY).
+#include "p2p_fp32_kernel.cuh"
+
+namespace photons {
+
+template <>
+int launch_p32_poly_deg<14>(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
+{
+    return launch_p32_close<GM_POLY, 14>(c, a, count, st);
+}
+
+}  // namespace photons

@@ -99,15 +99,14 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
         mbar_wait(&bars[st], (uint32_t)(k / N_STAGES) & 1u);
         const uint2 e = meta[st];
         const int ns = (int)(e.y & 0xffffu);
-        const int code = (int)((e.y >> 16) & 31u);
         const double4* src = reinterpret_cast<const double4*>(ring + (size_t)st * stage_bytes);
-        const bool per_pair = code == SHIFT_PER_PAIR;
+        const bool per_pair = (e.y & ENTRY_PER_PAIR) != 0;
         // image shift of this entry, moved onto the targets: d = (r_j + s L) - r_i = r_j - (r_i - s L)
         double sx = 0, sy = 0, sz = 0;
         if (!per_pair) {
-            sx = a.L * (double)(code % 3 - 1);
-            sy = a.L * (double)((code / 3) % 3 - 1);
-            sz = a.L * (double)(code / 9 - 1);
+            sx = a.L * (double)((int)((e.y >> 16) & 3u) - 1);
+            sy = a.L * (double)((int)((e.y >> 18) & 3u) - 1);
+            sz = a.L * (double)((int)((e.y >> 20) & 3u) - 1);
         }
         double px[T], py[T], pz[T], qx[T], qy[T], qz[T];
 #pragma unroll
