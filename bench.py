@@ -345,6 +345,59 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------ sweep (config 4)
+
+def run_sweep(args):
+    """BASELINE config 4's sweep: MAXLEAF 16/32/64/128 x g evaluated directly / from tables of 256, 512 (the
+    paper's), 1024, 4096 nodes / by the polynomial, fp32 vs mixed vs fp64.  Kernel-only times (CUDA events),
+    error against the oracle on sampled targets.  Prints a markdown table (see profiles/)."""
+    import torch
+    import oracle
+    from paper_2107_14008_b200 import binding as B
+    cfg = workloads.CONFIGS[args.config]
+    r_s, r_cut = geometry(cfg)
+    pos, mass = workloads.make(cfg)
+    tgt = workloads.sample_targets(cfg.n, args.sweep_targets, cfg.seed)
+    ref, cnt = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut, G=cfg.G)
+    rms = float(np.sqrt((ref ** 2).sum(axis=1).mean()))
+    in_cut_per_particle = cnt["pairs_in_cut"] / len(tgt)
+    d_pos = torch.from_numpy(pos.astype(np.float32)).cuda()
+    d_tgt = torch.from_numpy(tgt).cuda()
+    out = torch.empty((cfg.n, 3), dtype=torch.float64, device="cuda")
+    close = CLOSE_OVER_RCUT[cfg.kind] * r_cut
+    variants = [("fp32", "direct", {}), ("fp32", "poly", {})]
+    variants += [("fp32", "table", dict(table_nodes=n, table_level=2)) for n in (256, 512, 1024, 4096)]
+    variants += [("fp32", "table", dict(table_nodes=512, table_level=lv)) for lv in (0, 1, 3)]
+    variants += [("mixed", "direct", {}), ("mixed", "poly", {}), ("mixed", "table", dict(table_nodes=512, table_level=2))]
+    variants += [("fp64", "direct", {}), ("fp64", "table", dict(table_nodes=512, table_level=4)),
+                 ("fp64", "table", dict(table_nodes=4096, table_level=3))]
+    peak32 = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9
+    print(f"# sweep on {cfg.name}: N = {cfg.n}, N_PM = {cfg.n_pm}, close_pair_radius = {close / r_cut:g} r_cut, "
+          f"oracle on {len(tgt)} sampled targets (rms |a| = {rms:.4g}, {in_cut_per_particle:.0f} in-cut pairs per particle)\n")
+    print("| MAXLEAF | precision | g | evaluated pairs | kernel ms | pairs/s | in-cut pairs/s | paper-convention TFLOP/s (x51) "
+          "| % of fp32 peak (x51) | max err / rms |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for maxleaf in (16, 32, 64, 128):
+        for prec, g, extra in variants:
+            if args.sweep_quick and (maxleaf != 32 and (g == "table" and extra.get("table_nodes") != 512 or extra.get("table_level", 2) != 2)):
+                continue
+            params = headline_params(cfg, maxleaf=maxleaf, precision=prec, g_mode=g, close_pair_radius=close if prec != "fp64" else 0.0, **extra)
+            with B.Photons(**params) as ph:
+                ph.set_particles(d_pos, None)
+                ph.build_leaves()
+                ks = [ph.short_range_acc(out)["kernel_ms"] for _ in range(2 if prec != "fp64" else 1)]
+                st = ph.stats()
+            a = out[d_tgt].cpu().numpy()
+            err = float(np.sqrt(((a - ref) ** 2).sum(axis=1)).max() / rms)
+            ms = min(ks)
+            rate = st["pairs_evaluated"] / (ms * 1e-3)
+            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]"
+            print(f"| {maxleaf} | {prec} | {gname} | {st['pairs_evaluated']:.4g} | {ms:.2f} | {rate:.3e} | "
+                  f"{in_cut_per_particle * cfg.n / (ms * 1e-3):.3e} | {rate * PAPER_FLOPS_PER_PAIR / 1e12:.1f} | "
+                  f"{100 * rate * PAPER_FLOPS_PER_PAIR / peak32:.1f} | {err:.2e} |", flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -358,11 +411,16 @@ def main(argv=None):
     ap.add_argument("--streams", type=int, default=1)
     ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="MAXLEAF x g-mode x precision table instead of the bench line")
+    ap.add_argument("--sweep-targets", type=int, default=1000)
+    ap.add_argument("--sweep-quick", action="store_true", help="all table sizes/levels only at MAXLEAF 32")
     args = ap.parse_args(argv)
     if args.steps < 1 or args.warmup < 0:
         ap.error("--steps >= 1 and --warmup >= 0")
     if args.precision == "fp64" and args.g_mode == "poly":
         args.g_mode = "direct"
+    if args.sweep:
+        return run_sweep(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 
