@@ -378,6 +378,35 @@ def test_mixed_precision_on_unrounded_positions(B, oracle):
 
 # ----------------------------------------------------------- full size, in bench.py's launch configuration
 
+@pytest.mark.parametrize("cfg_id,n_targets", [(2, 2000), (3, 500)])
+def test_full_size_configs_2_and_3_sampled(B, oracle, cfg_id, n_targets):
+    """BASELINE configs 2 (128^3 clustered) and 3 (256^3 displaced grid) at full size in the headline launch
+    configuration (fp32, poly g, bench.CLOSE_OVER_RCUT), sampled targets; config 3 also in fp64."""
+    import bench
+    import torch
+    cfg = workloads.CONFIGS[cfg_id]
+    pos, mass = workloads.make(cfg)
+    r_s, r_cut = _geom(cfg)
+    tgt = workloads.sample_targets(cfg.n, n_targets, cfg.seed)
+    ref, cnt = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut)
+    if cfg_id == 3:   # homogeneous load: the closed-form neighbour count (4 pi / 3) 7.2^3 = 1563.5
+        assert cnt["pairs_in_cut"] / len(tgt) == pytest.approx(1563.5, rel=0.02)
+    dpos = torch.from_numpy(pos).cuda()
+    out = torch.empty((cfg.n, 3), dtype=torch.float64, device="cuda")
+    d_tgt = torch.from_numpy(tgt).cuda()
+    runs = [(bench.headline_params(cfg), TOL_FP32), (bench.headline_params(cfg, precision="mixed"), TOL_FP32),
+            (bench.headline_params(cfg, g_mode="table", table_nodes=512, table_level=2), TOL_TABLE)]
+    if cfg_id == 3:
+        runs.append((bench.headline_params(cfg, precision="fp64", g_mode="table", table_nodes=4096, table_level=3), TOL_FP64))
+    for params, tol in runs:
+        with B.Photons(**params) as ph:
+            ph.set_particles(dpos, None)
+            ph.build_leaves()
+            st = ph.short_range_acc(out)
+        assert _err(out[d_tgt].cpu().numpy(), ref) <= tol, params
+        assert st["n_leaves"] == cfg.n // cfg.maxleaf
+
+
 def test_full_size_config4_sampled(B, oracle):
     """BASELINE config 4 (N = 256^3 clustered, MAXLEAF 32) exactly as bench.py times it (fp32, poly g,
     close pairs on, device-resident input), checked on sampled targets the oracle computes one by one."""
