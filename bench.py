@@ -398,6 +398,46 @@ def run_sweep(args):
     return 0
 
 
+def run_table_study(args):
+    """Eq. 2 study (Fig. 2): every table size x Taylor level, fp32 and fp64, on one workload:
+    force error against the oracle and kernel time.  Prints a markdown table (see profiles/)."""
+    import torch
+    import oracle
+    from paper_2107_14008_b200 import binding as B
+    cfg = workloads.CONFIGS[args.config]
+    r_s, r_cut = geometry(cfg)
+    pos, mass = workloads.make(cfg)
+    tgt = workloads.sample_targets(cfg.n, args.sweep_targets, cfg.seed)
+    ref, _ = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut, G=cfg.G)
+    rms = float(np.sqrt((ref ** 2).sum(axis=1).mean()))
+    d_pos = torch.from_numpy(pos.astype(np.float32)).cuda()
+    d_tgt = torch.from_numpy(tgt).cuda()
+    out = torch.empty((cfg.n, 3), dtype=torch.float64, device="cuda")
+    close = CLOSE_OVER_RCUT[cfg.kind] * r_cut
+    print(f"# Eq. 2 table study on {cfg.name}: N = {cfg.n}, MAXLEAF = {cfg.maxleaf}, oracle on {len(tgt)} sampled targets\n")
+    print("| precision | nodes | level | max table error of T (fp64, oracle/table.py) | max err / rms of the force | kernel ms | pairs/s |")
+    print("|---|---|---|---|---|---|---|")
+    xq = np.linspace(0.0, 3.0, 200001)
+    t_exact = oracle.oracle_T(np.linspace(0.0, 3.0, 2001))
+    for prec in ("fp32", "fp64"):
+        for nodes in (256, 512, 1024, 4096):
+            for level in range(0, 4 if prec == "fp32" else 5):
+                tab_err = float(np.abs(oracle.eval_table(np.linspace(0.0, 3.0, 2001), nodes, level) - t_exact).max())
+                params = headline_params(cfg, precision=prec, g_mode="table", table_nodes=nodes, table_level=level,
+                                         close_pair_radius=close if prec != "fp64" else 0.0)
+                with B.Photons(**params) as ph:
+                    ph.set_particles(d_pos, None)
+                    ph.build_leaves()
+                    ks = [ph.short_range_acc(out)["kernel_ms"] for _ in range(2 if prec != "fp64" else 1)]
+                    st = ph.stats()
+                a = out[d_tgt].cpu().numpy()
+                err = float(np.sqrt(((a - ref) ** 2).sum(axis=1)).max() / rms)
+                print(f"| {prec} | {nodes} | T[{level}] | {tab_err:.2e} | {err:.2e} | {min(ks):.2f} | "
+                      f"{st['pairs_evaluated'] / (min(ks) * 1e-3):.3e} |", flush=True)
+    del xq
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -412,6 +452,7 @@ def main(argv=None):
     ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="MAXLEAF x g-mode x precision table instead of the bench line")
+    ap.add_argument("--table-study", action="store_true", help="Eq. 2: table size x Taylor level, fp32 and fp64")
     ap.add_argument("--sweep-targets", type=int, default=1000)
     ap.add_argument("--sweep-quick", action="store_true", help="all table sizes/levels only at MAXLEAF 32")
     args = ap.parse_args(argv)
@@ -421,6 +462,8 @@ def main(argv=None):
         args.g_mode = "direct"
     if args.sweep:
         return run_sweep(args)
+    if args.table_study:
+        return run_table_study(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 
