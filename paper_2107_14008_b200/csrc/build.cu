@@ -118,15 +118,16 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
     vals[q] = (uint32_t)q;
 }
 
-__device__ __forceinline__ void cta_bitonic_sort(unsigned long long* key, int n2)
+// sorts every aligned window of kmax keys ascending (kmax = n2: the whole array)
+__device__ __forceinline__ void cta_bitonic_sort(unsigned long long* key, int n2, int kmax)
 {
-    for (int k = 2; k <= n2; k <<= 1) {
+    for (int k = 2; k <= kmax; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
             for (int t = threadIdx.x; t < (n2 >> 1); t += blockDim.x) {
                 const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // the lower index of the t-th pair
                 const int l = i | j;
                 const unsigned long long a = key[i], b = key[l];
-                const bool up = (i & k) == 0;
+                const bool up = (i & k) == 0 || k == kmax;
                 if ((a > b) == up) { key[i] = b; key[l] = a; }
             }
             __syncthreads();
@@ -186,7 +187,8 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
             key[e] = k;
         }
         __syncthreads();
-        cta_bitonic_sort(key, n2);
+        // when the node holds a power of two of particles its sub-nodes are aligned windows: sort them separately
+        cta_bitonic_sort(key, n2, size == n2 ? (n2 >> sl) : n2);
         // apply the order: read through the sorted local indices, then write back
         float4 tmp[ORB_CTA_MAX / ORB_CTA_THREADS];
         for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) tmp[r] = cur[(int)(key[e] & 0xfffu)];
@@ -283,7 +285,7 @@ struct ListArgs {
     long long n_leaves;
     int depth, maxleaf, chunk_max;
     double L, rcut;
-    const double *node_lo, *node_hi;
+    const float4* box;            // 2 per tree node (heap order): {centre, .}, {half-width rounded up, .}
     const int* leaf_cnt;
     const long long* chunk_ptr;   // pass 2
     uint2* chunks;                // pass 2
@@ -298,13 +300,16 @@ __global__ void list_kernel(ListArgs a)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= a.n_leaves) return;
-    const long long leaf0 = a.n_leaves - 1;   // heap index of leaf 0
-    double tl[3], th[3];
-    for (int x = 0; x < 3; ++x) { tl[x] = a.node_lo[3 * (leaf0 + i) + x]; th[x] = a.node_hi[3 * (leaf0 + i) + x]; }
-    const double rc2 = a.rcut * a.rcut;
+    const int leaf0 = (int)(a.n_leaves - 1);   // heap index of leaf 0
+    // fp32 walk on {centre, half-width} boxes whose half-widths were rounded up (node_box32_kernel) and with a
+    // slack of 1e-6 L on every gap: it can only accept more than the exact test would, never less.
+    const float4 tc = a.box[2 * (size_t)(leaf0 + i)], thw = a.box[2 * (size_t)(leaf0 + i) + 1];
+    const float Lf = (float)a.L, invL = (float)(1.0 / a.L), slack = 1e-6f * Lf;
+    const float rc2 = (float)(a.rcut * a.rcut) * (1.0f + 1e-6f);
+    const float amb = Lf - 2.0f * (float)a.rcut;      // ambiguous image iff 2 (hw_i + hw_j) >= amb  (A10)
     const int my_cnt = a.leaf_cnt[i];
 
-    long long stack[40];
+    int stack[40];
     int sp = 0;
     stack[sp++] = 0;
     long long run_first = -1, run_n = 0, n_chunks = 0, n_pairs = 0, n_eval = 0, work = 0;
@@ -317,22 +322,23 @@ __global__ void list_kernel(ListArgs a)
     const int max_leaves_per_chunk = a.chunk_max / a.maxleaf;
 
     while (sp) {
-        const long long node = stack[--sp];
-        double g2 = 0;
-        int code = 0, shl = 16;       // the three shift fields of entry_pack, without the slot count
+        const int node = stack[--sp];
+        const float4 nc = __ldg(&a.box[2 * (size_t)node]), nhw = __ldg(&a.box[2 * (size_t)node + 1]);
+        float g2 = 0.f;
+        int code = 0;                 // the three shift fields of entry_pack, without the slot count
         bool ambiguous = false;
-        for (int x = 0; x < 3; ++x) {
-            const double nl = a.node_lo[3 * node + x], nh = a.node_hi[3 * node + x];
-            const double hw = 0.5 * ((nh - nl) + (th[x] - tl[x]));
-            double dc = 0.5 * ((nl + nh) - (tl[x] + th[x]));
-            const double img = rint(dc / a.L);      // source is moved by -img box lengths
-            dc -= a.L * img;
-            const double gap = fmax(0.0, fabs(dc) - hw);
-            g2 += gap * gap;
-            code |= (1 - (int)img) << shl;
-            shl += 2;
-            // the image is unique for every pair inside r_cut iff 2 r_cut + extents < L (A10)
-            if (2.0 * a.rcut + 2.0 * hw >= a.L) ambiguous = true;
+        {
+            const float dcs[3] = {nc.x - tc.x, nc.y - tc.y, nc.z - tc.z};
+            const float hws[3] = {nhw.x + thw.x, nhw.y + thw.y, nhw.z + thw.z};
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const float img = rintf(dcs[x] * invL);      // source is moved by -img box lengths
+                const float dc = fmaf(-Lf, img, dcs[x]);
+                const float gap = fmaxf(0.f, fabsf(dc) - hws[x] - slack);
+                g2 = fmaf(gap, gap, g2);
+                code |= (1 - (int)img) << (16 + 2 * x);
+                if (2.0f * hws[x] >= amb) ambiguous = true;
+            }
         }
         if (!(g2 < rc2)) continue;
         if (node < leaf0) {               // internal: right child first so the left one is popped first
@@ -369,6 +375,21 @@ __global__ void list_kernel(ListArgs a)
         atomicAdd(&a.totals[0], (unsigned long long)n_pairs);
         atomicAdd(&a.totals[1], (unsigned long long)n_eval);
     }
+}
+
+// fp32 boxes for the list walk: centre rounded to nearest, half-width rounded up and widened by the centre's rounding
+__global__ void node_box32_kernel(long long n_nodes, const double* __restrict__ lo, const double* __restrict__ hi, float4* __restrict__ box)
+{
+    long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= n_nodes) return;
+    float c[3], h[3];
+    for (int a = 0; a < 3; ++a) {
+        const double cd = 0.5 * (lo[3 * k + a] + hi[3 * k + a]);
+        c[a] = (float)cd;
+        h[a] = __double2float_ru(0.5 * (hi[3 * k + a] - lo[3 * k + a]) + fabs(cd - (double)c[a]));
+    }
+    box[2 * k] = make_float4(c[0], c[1], c[2], 0.f);
+    box[2 * k + 1] = make_float4(h[0], h[1], h[2], 0.f);
 }
 
 // one warp per leaf: stash -> CSR for the lists that fitted into the stash
@@ -526,7 +547,14 @@ int build_leaves_impl(Ctx* c)
     ListArgs la{};
     la.n_leaves = n_leaves; la.depth = depth; la.maxleaf = M; la.chunk_max = c->p.chunk_max;
     la.L = c->p.boxsize; la.rcut = c->r_cut;
-    la.node_lo = c->d_node_lo; la.node_hi = c->d_node_hi; la.leaf_cnt = c->d_leaf_cnt;
+    {
+        float4* box = nullptr;
+        PH_WS(box, float4, WS_NODE_BOX32, 2 * n_nodes);
+        node_box32_kernel<<<blocks_for(n_nodes, tb), tb, 0, st>>>(n_nodes, c->d_node_lo, c->d_node_hi, box);
+        ++c->launches;
+        la.box = box;
+    }
+    la.leaf_cnt = c->d_leaf_cnt;
     la.chunk_ptr = nullptr; la.chunks = nullptr; la.n_chunks_of = d_nch; la.totals = d_tot; la.work_of = d_work;
     la.stash_cap = LIST_STASH;
     PH_WS(la.stash, uint2, WS_LIST_STASH, n_leaves * LIST_STASH);

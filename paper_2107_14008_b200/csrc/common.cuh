@@ -43,7 +43,7 @@ constexpr int POLY_MAX_DEG = 20;
 enum WsSlot {
     WS_POS, WS_MASS, WS_IN_POS, WS_IN_MASS, WS_FLAG, WS_OUT,
     WS_PERM, WS_ORB_P0, WS_ORB_P1, WS_ORB_KEYS, WS_ORB_KEYS2, WS_ORB_VALS, WS_ORB_VALS2, WS_ORB_LO, WS_ORB_HI, WS_CUB_TMP,
-    WS_LEAF_CNT, WS_NODE_LO, WS_NODE_HI, WS_LEAF_CTR, WS_SLOT_SRC, WS_P64, WS_P32,
+    WS_LEAF_CNT, WS_NODE_LO, WS_NODE_HI, WS_NODE_BOX32, WS_LEAF_CTR, WS_SLOT_SRC, WS_P64, WS_P32,
     WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_LIST_STASH, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
     WS_COUNT
 };
