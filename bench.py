@@ -55,6 +55,9 @@ def flops_per_pair(g_mode: str, poly_degree: int = POLY_DEGREE) -> float:
         return 2.0 * 9 + 6 + 10 + 1
     return 51.0                # direct: the paper's convention; erfcf/expf are not itemised
 PAPER_FLOPS_PER_PAIR = 51.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the headline kernel, from the committed
+# `ncu --set full` capture (profiles/r1_p2p_fp32_poly12_ncu_full.md): config 4, MAXLEAF 32, fp32, poly.
+NCU_TRAFFIC_BYTES = {("c4_clustered_256", 32, "fp32", "poly"): 20.170781e9 + 0.670968576e9}
 
 
 def geometry(cfg):
@@ -298,7 +301,9 @@ def run_ours(args):
         achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
         roofline = {
             "bound": "alu", "kernel": "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-            "frac": achieved_tf / peak_tf, "traffic": None,
+            "frac": achieved_tf / peak_tf,
+            "traffic": NCU_TRAFFIC_BYTES.get((cfg0.name, params["maxleaf"], args.precision, args.g_mode)),
+            "traffic_unit": "bytes per launch (ncu dram read + write; the bound is ALU, not HBM)",
             "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); "
                            "MEASURED_PEAKS.json holds no FP32 vector peak",
             "flops_per_pair": fpp, "kernel_ms": kernel_ms, "kernel_pairs_per_s": pairs / (kernel_ms * 1e-3),
