@@ -100,8 +100,9 @@ __device__ __forceinline__ int widest_axis(const float ext[3])
     return axis;
 }
 
+template <typename Key>     // 32-bit keys while node index and coordinate fit (levels 0..8), 64-bit after
 __global__ void orb_key_kernel(long long n, int level, const float4* __restrict__ P, const int* __restrict__ lo,
-                               const int* __restrict__ hi, unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals)
+                               const int* __restrict__ hi, Key* __restrict__ keys, uint32_t* __restrict__ vals)
 {
     long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (q >= n) return;
@@ -114,7 +115,7 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
     // monotone map of [lo, hi] onto 24-bit integers
     const float u = ext[axis] > 0.f ? (x - l[axis]) / ext[axis] : 0.f;
     const unsigned f = (unsigned)fminf(u * 16777215.0f, 16777215.0f);
-    keys[q] = ((unsigned long long)seg << 24) | f;
+    keys[q] = (Key)(((unsigned long long)seg << 24) | f);
     vals[q] = (uint32_t)q;
 }
 
@@ -458,6 +459,12 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         PH_WS(hi, int, WS_ORB_HI, 3LL << L0);
         size_t tmp_bytes = 0;
         PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + L0, st));
+        {
+            size_t need32 = 0;
+            PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, need32, reinterpret_cast<uint32_t*>(keys), reinterpret_cast<uint32_t*>(keys2),
+                                                          vals, vals2, (int)n, 0, 32, st));
+            tmp_bytes = std::max(tmp_bytes, need32);
+        }
         void* tmp = workspace(c, WS_CUB_TMP, tmp_bytes);
         if (!tmp) return PHOTONS_ENOMEM;
         fill_int_kernel<<<1, 32, 0, st>>>(3, lo, 0x7fffffff);
@@ -465,9 +472,16 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, 0, nullptr, P_cur, nullptr, lo, hi);
         c->launches += 3;
         for (int level = 0; level < L0; ++level) {
-            orb_key_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, keys, vals);
+            if (24 + level <= 32) {
+                uint32_t* k32 = reinterpret_cast<uint32_t*>(keys);
+                uint32_t* k32b = reinterpret_cast<uint32_t*>(keys2);
+                orb_key_kernel<uint32_t><<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, k32, vals);
+                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k32, k32b, vals, vals2, (int)n, 0, 24 + level, st));
+            } else {
+                orb_key_kernel<unsigned long long><<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, keys, vals);
+                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + level, st));
+            }
             ++c->launches;
-            PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + level, st));
             const bool more = level + 1 < L0;   // the next level's boxes, reduced while the order is applied
             if (more) {
                 const long long nb = 3LL << (level + 1);

@@ -15,7 +15,8 @@
 #include "pipeline.cuh"
 
 #ifndef PHOTONS_UNROLL_T1
-#define PHOTONS_UNROLL_T1 4   // source pairs per loop iteration with one target per lane (measured: 4 beats 2 by 3 %)
+#define PHOTONS_UNROLL_T1 8   // source pairs per loop iteration with one target per lane (measured on config 4:
+                              // 2: 103.2 ms, 4: 96.3 ms, 8: 94.4 ms)
 #endif
 #ifndef PHOTONS_UNROLL_T2
 #define PHOTONS_UNROLL_T2 2   // ... with two targets per lane
@@ -345,7 +346,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                 }
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
                 // U source pairs x T targets = NCH independent chains per iteration
-                constexpr int U = T == 1 ? PHOTONS_UNROLL_T1 : T == 2 ? PHOTONS_UNROLL_T2 : 1;
+                // (with lane groups the leaf's np = maxleaf/2 source pairs are shared out, so fewer fit in one iteration)
+                constexpr int U = T == 1 ? (HS == 1 ? PHOTONS_UNROLL_T1 : PHOTONS_UNROLL_T1 / 2) : T == 2 ? PHOTONS_UNROLL_T2 : 1;
                 constexpr int NCH = U * T;
                 auto step = [&](const int p, const bool with_seam) {
                     float2 dx[NCH], dy[NCH], dz[NCH], r2[NCH], gm[NCH], w[NCH];
