@@ -89,6 +89,9 @@ typedef struct {
                                  into 32 T / maxleaf groups that take alternate source pairs); 0 = default.
                                  Available: maxleaf 16: 1, 2; 32: 1, 2; 64: 2; 128: 4 */
     int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12) */
+    int periodic;             /* 1 = periodic cube of side boxsize, minimum image (default; north_star);
+                                 0 = isolated boundaries: no images, positions are not wrapped,
+                                 boxsize only sets r_s = rs_over_cell * boxsize / n_pm */
 } photons_params;
 
 typedef struct {
@@ -106,7 +109,7 @@ typedef struct {
 } photons_stats;
 
 /* Fill *p with the paper's defaults: boxsize 1, n_pm 32, rs_over_cell 1.2, rcut_over_rs 6, G 1, maxleaf 32,
- * FP32, G_POLY, table 512/level 2, 1 stream, device 0, close pairs off, chunk_max default. */
+ * FP32, G_POLY, table 512/level 2, 1 stream, device 0, close pairs off, chunk_max default, periodic. */
 void photons_default_params(photons_params* p);
 
 /* Validate parameters, select the device, create streams, build the g table (TABLE mode; fp64 on the

@@ -82,7 +82,7 @@ def _call(pos, mass, tgt, boxsize, r_s, r_cut, G):
 
 
 def p2p(pos, mass, *, boxsize, r_s, r_cut, G=1.0):
-    """Full O(N^2) sum: acc[n,3] and counters."""
+    """Full O(N^2) sum: acc[n,3] and counters.  boxsize <= 0 means isolated boundaries (no images)."""
     return _call(pos, mass, None, boxsize, r_s, r_cut, G)
 
 

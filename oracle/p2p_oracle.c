@@ -7,7 +7,8 @@
  *
  *   a_i = G * sum_{j != i, 0 < |d_ij| < r_cut}  m_j * d_ij * T(|d_ij|; r_s) / |d_ij|^3
  *
- *   d_ij = minimum image of (r_j - r_i) in the periodic cube of side L     (north_star; A10)
+ *   d_ij = minimum image of (r_j - r_i) in the periodic cube of side L     (north_star; A10);
+ *          with L <= 0 the boundaries are isolated: d_ij = r_j - r_i
  *   T(r; r_s) = erfc(r / 2 r_s) + r / (r_s sqrt(pi)) * exp(-r^2 / 4 r_s^2)    (Eq. 1)
  *   sign: dx = pos_j - pos_i and a += grav*dx, i.e. attraction towards j     (Alg. 2;
  *         L55 "F_s = -r/r^3 T" with r = r_i - r_j; A3)
@@ -73,9 +74,11 @@ void oracle_p2p(long long n, const double *pos, const double *mass,
             double dx = pos[3 * j] - xi;
             double dy = pos[3 * j + 1] - yi;
             double dz = pos[3 * j + 2] - zi;
-            dx -= L * nearbyint(dx / L);               /* minimum image, per axis */
-            dy -= L * nearbyint(dy / L);
-            dz -= L * nearbyint(dz / L);
+            if (L > 0.0) {                             /* L <= 0: isolated boundaries, no images */
+                dx -= L * nearbyint(dx / L);           /* minimum image, per axis */
+                dy -= L * nearbyint(dy / L);
+                dz -= L * nearbyint(dz / L);
+            }
             const double r2 = dx * dx + dy * dy + dz * dz;
             if (r2 > 0.0 && r2 < rcut2) {
                 const double r = sqrt(r2);

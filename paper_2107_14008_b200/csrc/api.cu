@@ -55,7 +55,7 @@ static double now_ms()
 
 // wrap into [0, L), flag non-finite values; src is fp64 or fp32
 template <typename Tin>
-__global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Tin* __restrict__ mass, double L,
+__global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Tin* __restrict__ mass, double L, int periodic,
                               double default_mass, double* __restrict__ opos, double* __restrict__ omass,
                               int* __restrict__ bad)
 {
@@ -65,9 +65,11 @@ __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Ti
     for (int a = 0; a < 3; ++a) {
         double x = (double)pos[3 * i + a];
         if (!isfinite(x)) { ok = false; x = 0.0; }
-        x -= L * floor(x / L);
-        if (x >= L) x -= L;      // x/L rounding can leave x == L
-        if (x < 0.0) x = 0.0;
+        if (periodic) {
+            x -= L * floor(x / L);
+            if (x >= L) x -= L;      // x/L rounding can leave x == L
+            if (x < 0.0) x = 0.0;
+        }
         opos[3 * i + a] = x;
     }
     double m = mass ? (double)mass[i] : default_mass;
@@ -117,6 +119,7 @@ void photons_default_params(photons_params* p)
     p->warps_per_leaf = 0;
     p->targets_per_lane = 0;
     p->poly_degree = 0;
+    p->periodic = 1;
 }
 
 static int create_fail(char* err_buf, int err_len, int code, const char* msg)
@@ -164,7 +167,8 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
 
     const double r_s = p.rs_over_cell * p.boxsize / p.n_pm;
     const double r_cut = p.rcut_over_rs * r_s;
-    if (!(r_cut < 0.5 * p.boxsize)) return create_fail(err_buf, err_len, PHOTONS_EBOX, "r_cut >= boxsize/2: minimum image is not unique");
+    if (p.periodic != 0 && p.periodic != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "periodic must be 0 or 1");
+    if (p.periodic && !(r_cut < 0.5 * p.boxsize)) return create_fail(err_buf, err_len, PHOTONS_EBOX, "r_cut >= boxsize/2: minimum image is not unique");
     if (p.close_pair_radius >= r_cut) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be < r_cut");
 
     int ndev = 0;
@@ -252,9 +256,9 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     const int tb = 256;
     const unsigned nb = (unsigned)((n + tb - 1) / tb);
     if (dtype == PHOTONS_DTYPE_F64)
-        intake_kernel<double><<<nb, tb, 0, st>>>(n, (const double*)src_pos, (const double*)src_mass, c->p.boxsize, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
+        intake_kernel<double><<<nb, tb, 0, st>>>(n, (const double*)src_pos, (const double*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
     else
-        intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
+        intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
     ++c->launches;
     int bad = 0;
     cudaError_t e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);

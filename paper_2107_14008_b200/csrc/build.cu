@@ -49,7 +49,7 @@ __global__ void fill_int_kernel(long long n, int* p, int v)
 }
 
 // P_out[q] = P_in[src[q]] (src == nullptr: identity), and the bounding boxes of the level-`level` nodes as
-// fp32 bit patterns (positions are >= 0, so the integer order of the bits is the float order).  Reduced per
+// order-preserving integers (f2ord).  Reduced per
 // warp and, when the whole block sits in one node (the upper levels), per block, before the global atomics.
 __global__ void __launch_bounds__(256) orb_gather_bbox_kernel(long long n, int level, const uint32_t* __restrict__ src,
                                                               const float4* __restrict__ P_in, float4* __restrict__ P_out,
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(256) orb_gather_bbox_kernel(long long n, int l
     const long long q_first = blockIdx.x * (long long)blockDim.x;
     const long long q_last = min(q_first + blockDim.x, n) - 1;
     const bool block_uniform = seg_of(n, level, q_first) == seg_of(n, level, q_last);
-    const int v[3] = {__float_as_int(p.x), __float_as_int(p.y), __float_as_int(p.z)};
+    const int v[3] = {f2ord(p.x), f2ord(p.y), f2ord(p.z)};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long seg0 = __shfl_sync(0xffffffffu, seg, 0);
     const bool warp_uniform = __all_sync(0xffffffffu, seg == seg0);
@@ -108,7 +108,7 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
     if (q >= n) return;
     const long long seg = seg_of(n, level, q);
     float l[3], ext[3];
-    for (int a = 0; a < 3; ++a) { l[a] = __int_as_float(lo[3 * seg + a]); ext[a] = __int_as_float(hi[3 * seg + a]) - l[a]; }
+    for (int a = 0; a < 3; ++a) { l[a] = ord2f(lo[3 * seg + a]); ext[a] = ord2f(hi[3 * seg + a]) - l[a]; }
     const int axis = widest_axis(ext);
     const float4 p = P[q];
     const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
@@ -155,14 +155,14 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
     for (int level = L0; level < depth; ++level) {
         const int sl = level - L0;                   // nodes of this CTA at this level: 2^sl (<= 128)
         const int nsub = 1 << sl;
-        for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { blo[i] = 0x7fffffff; bhi[i] = 0; }
+        for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { blo[i] = 0x7fffffff; bhi[i] = (int)0x80000000; }
         __syncthreads();
         for (int e0 = 0; e0 < size; e0 += blockDim.x) {       // whole warps enter: the votes below need all lanes
             const int e = e0 + threadIdx.x;
             const bool live = e < size;
             const int sub = (int)seg_of(size, sl, live ? e : size - 1);
             const float4 p = cur[live ? e : size - 1];
-            const int v[3] = {__float_as_int(p.x), __float_as_int(p.y), __float_as_int(p.z)};
+            const int v[3] = {f2ord(p.x), f2ord(p.y), f2ord(p.z)};
             const int sub0 = __shfl_sync(0xffffffffu, sub, 0);
             if (__all_sync(0xffffffffu, sub == sub0)) {
                 for (int a = 0; a < 3; ++a) {
@@ -179,11 +179,11 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
             if (e < size) {
                 const int sub = (int)seg_of(size, sl, e);
                 float ext[3];
-                for (int a = 0; a < 3; ++a) ext[a] = __int_as_float(bhi[3 * sub + a]) - __int_as_float(blo[3 * sub + a]);
+                for (int a = 0; a < 3; ++a) ext[a] = ord2f(bhi[3 * sub + a]) - ord2f(blo[3 * sub + a]);
                 const int axis = widest_axis(ext);
                 const float4 p = cur[e];
                 const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
-                k = ((unsigned long long)sub << 44) | ((unsigned long long)(unsigned)__float_as_int(x) << 12) | (unsigned)e;
+                k = ((unsigned long long)sub << 44) | ((unsigned long long)((unsigned)f2ord(x) ^ 0x80000000u) << 12) | (unsigned)e;
             }
             key[e] = k;
         }
@@ -284,7 +284,7 @@ constexpr int LIST_STASH = 128;   // list entries per leaf kept from the countin
 
 struct ListArgs {
     long long n_leaves;
-    int depth, maxleaf, chunk_max;
+    int depth, maxleaf, chunk_max, periodic;
     double L, rcut;
     const float4* box;            // 2 per tree node (heap order): {centre, .}, {half-width rounded up, .}
     const int* leaf_cnt;
@@ -333,12 +333,12 @@ __global__ void list_kernel(ListArgs a)
             const float hws[3] = {nhw.x + thw.x, nhw.y + thw.y, nhw.z + thw.z};
 #pragma unroll
             for (int x = 0; x < 3; ++x) {
-                const float img = rintf(dcs[x] * invL);      // source is moved by -img box lengths
+                const float img = a.periodic ? rintf(dcs[x] * invL) : 0.f;      // source is moved by -img box lengths
                 const float dc = fmaf(-Lf, img, dcs[x]);
                 const float gap = fmaxf(0.f, fabsf(dc) - hws[x] - slack);
                 g2 = fmaf(gap, gap, g2);
                 code |= (1 - (int)img) << (16 + 2 * x);
-                if (2.0f * hws[x] >= amb) ambiguous = true;
+                if (a.periodic && 2.0f * hws[x] >= amb) ambiguous = true;
             }
         }
         if (!(g2 < rc2)) continue;
@@ -468,7 +468,7 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         void* tmp = workspace(c, WS_CUB_TMP, tmp_bytes);
         if (!tmp) return PHOTONS_ENOMEM;
         fill_int_kernel<<<1, 32, 0, st>>>(3, lo, 0x7fffffff);
-        fill_int_kernel<<<1, 32, 0, st>>>(3, hi, 0);
+        fill_int_kernel<<<1, 32, 0, st>>>(3, hi, (int)0x80000000);
         orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, 0, nullptr, P_cur, nullptr, lo, hi);
         c->launches += 3;
         for (int level = 0; level < L0; ++level) {
@@ -486,7 +486,7 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
             if (more) {
                 const long long nb = 3LL << (level + 1);
                 fill_int_kernel<<<blocks_for(nb, tb), tb, 0, st>>>(nb, lo, 0x7fffffff);
-                fill_int_kernel<<<blocks_for(nb, tb), tb, 0, st>>>(nb, hi, 0);
+                fill_int_kernel<<<blocks_for(nb, tb), tb, 0, st>>>(nb, hi, (int)0x80000000);
                 c->launches += 2;
             }
             orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, level + 1, vals2, P_cur, P_alt, more ? lo : nullptr, hi);
@@ -560,7 +560,7 @@ int build_leaves_impl(Ctx* c)
     PH_CUDA_BUILD(cudaMemsetAsync(d_nch, 0, sizeof(long long) * (n_leaves + 1), st));
     ListArgs la{};
     la.n_leaves = n_leaves; la.depth = depth; la.maxleaf = M; la.chunk_max = c->p.chunk_max;
-    la.L = c->p.boxsize; la.rcut = c->r_cut;
+    la.L = c->p.boxsize; la.rcut = c->r_cut; la.periodic = c->p.periodic;
     {
         float4* box = nullptr;
         PH_WS(box, float4, WS_NODE_BOX32, 2 * n_nodes);

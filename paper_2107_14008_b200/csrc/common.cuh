@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <cstdio>
+#include <cstring>
 #include <string>
 #include <vector>
 
@@ -116,6 +117,21 @@ int make_poly(Ctx* c);
 // out = device buffer in caller order (n x 3, fp64 or fp32 as out_f32 says)
 int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st);
 int launch_p2p_fp32(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st);
+
+// float <-> int whose signed integer order is the float order (negative coordinates occur with isolated boundaries)
+__host__ __device__ inline int f2ord(float f)
+{
+    int b;
+    memcpy(&b, &f, 4);
+    return b ^ ((b >> 31) & 0x7fffffff);
+}
+__host__ __device__ inline float ord2f(int o)
+{
+    o ^= (o >> 31) & 0x7fffffff;
+    float f;
+    memcpy(&f, &o, 4);
+    return f;
+}
 
 // first sorted position of segment k at tree level `level` when n particles are bisected with the
 // left child taking floor(size/2) (A13)

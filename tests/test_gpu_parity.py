@@ -292,6 +292,31 @@ def test_perfect_lattice_has_zero_force(B):
     assert np.abs(out).max() <= 1e-12 * scale
 
 
+def test_isolated_boundaries(B, oracle):
+    """periodic = 0: no images, no wrapping, negative coordinates; oracle with boxsize <= 0."""
+    rng = np.random.default_rng(77)
+    n = 20000
+    n_pm = 32
+    r_s = 1.2 / n_pm
+    r_cut = 6 * r_s
+    # a blob that straddles the origin and the faces of the nominal unit box
+    pos = (rng.normal(0.0, 0.35, (n, 3)) + np.array([0.1, 0.9, -0.2])).astype(np.float32).astype(np.float64)
+    mass = rng.uniform(0.5, 1.5, n) / n
+    ref, _ = oracle.p2p(pos, mass, boxsize=0.0, r_s=r_s, r_cut=r_cut)
+    per, _ = oracle.p2p(np.mod(pos, 1.0), mass, boxsize=1.0, r_s=r_s, r_cut=r_cut)
+    assert _err(per, ref) > 1e-3                    # the periodic answer really is a different one
+    for prec, g, tol, kw in (("fp64", "direct", TOL_FP64, {}), ("fp32", "poly", TOL_FP32, dict(close_pair_radius=0.02 * r_cut)),
+                             ("mixed", "poly", TOL_FP32, dict(close_pair_radius=0.02 * r_cut)),
+                             ("fp32", "table", TOL_TABLE, dict(close_pair_radius=0.02 * r_cut)),
+                             ("fp32", "direct", TOL_FP32, dict(close_pair_radius=0.02 * r_cut, maxleaf=16))):
+        out, _ = B.short_range_acc(pos, mass, n_pm=n_pm, periodic=0, precision=prec, g_mode=g, **kw)
+        assert _err(out, ref) <= tol, (prec, g)
+    # isolated mode has no r_cut < L/2 requirement
+    out, _ = B.short_range_acc(pos[:50] * 0.01, mass[:50], boxsize=1.0, n_pm=8, periodic=0, precision="fp64", g_mode="direct")
+    ref8, _ = oracle.p2p(pos[:50] * 0.01, mass[:50], boxsize=0.0, r_s=1.2 / 8, r_cut=6 * 1.2 / 8)
+    assert _err(out, ref8) <= TOL_FP64
+
+
 # ---------------------------------------------------------------------------- error behaviour (ABI)
 
 def test_abi_errors(B):

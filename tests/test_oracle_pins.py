@@ -326,3 +326,38 @@ def test_paper_perf_accounting_is_self_consistent():
     assert avg / g["machine_peak_tflops"] == pytest.approx(g["average_fraction_printed"], abs=0.01)
     # printed 48 %; plain arithmetic gives 49.3 % (A17)
     assert peak / g["machine_peak_tflops"] == pytest.approx(0.493, abs=0.002)
+
+
+# ------------------------------------------------------------- isolated boundaries
+
+def test_isolated_two_body_has_no_image_force(oracle):
+    # across the seam of the unit box the periodic pair is close, the isolated pair is far beyond the cut
+    n_pm = 32
+    r_s = 1.2 / n_pm
+    pos = np.array([[0.99, 0.5, 0.5], [0.02, 0.5, 0.5]])
+    mass = np.array([1.0, 2.0])
+    per, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=6 * r_s)
+    iso, cnt = oracle.p2p(pos, mass, boxsize=0.0, r_s=r_s, r_cut=6 * r_s)
+    assert per[0, 0] > 0 and np.all(iso == 0.0) and cnt["pairs_in_cut"] == 0
+    # a close isolated pair, negative coordinates allowed: closed form
+    d = 0.04
+    pos = np.array([[-0.3, 0.1, -2.0], [-0.3 + d, 0.1, -2.0]])
+    iso, _ = oracle.p2p(pos, mass, boxsize=0.0, r_s=r_s, r_cut=6 * r_s)
+    g = float(T_mp(d / (2 * r_s)))
+    assert iso[0, 0] == pytest.approx(2.0 * g / d ** 2, rel=1e-13)
+    assert iso[1, 0] == pytest.approx(-1.0 * g / d ** 2, rel=1e-13)
+
+
+def test_isolated_equals_periodic_far_from_the_faces(oracle):
+    # a blob that stays more than r_cut away from every face of the box feels no images: both modes agree bitwise
+    rng = np.random.default_rng(11)
+    n_pm = 32
+    r_s = 1.2 / n_pm
+    pos = 0.35 + 0.3 * rng.random((400, 3))
+    mass = rng.uniform(0.5, 1.5, 400)
+    per, c1 = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=6 * r_s)
+    iso, c2 = oracle.p2p(pos, mass, boxsize=0.0, r_s=r_s, r_cut=6 * r_s)
+    assert np.array_equal(per, iso) and c1 == c2
+    # and Newton's third law holds in the isolated mode too
+    tot = (mass[:, None] * iso).sum(axis=0)
+    assert np.abs(tot).max() <= 1e-12 * (mass[:, None] * np.abs(iso)).sum()
