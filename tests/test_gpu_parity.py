@@ -432,6 +432,29 @@ def test_full_size_configs_2_and_3_sampled(B, oracle, cfg_id, n_targets):
         assert st["n_leaves"] == cfg.n // cfg.maxleaf
 
 
+def test_full_size_config5_mixed_4_streams(B, oracle):
+    """BASELINE config 5: N = 512^3 clustered, N_PM 512, MAXLEAF 32, mixed precision, leaf batches over 4 CUDA
+    streams; oracle on sampled targets (128 here; bench-side studies use more)."""
+    import bench
+    import torch
+    cfg = workloads.CONFIGS[5]
+    pos, mass = workloads.make(cfg)
+    r_s, r_cut = _geom(cfg)
+    tgt = workloads.sample_targets(cfg.n, 128, cfg.seed)
+    ref, _ = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut)
+    dpos = torch.from_numpy(pos.astype(np.float32)).cuda()       # flavour F: exact in fp32
+    del pos
+    out = torch.empty((cfg.n, 3), dtype=torch.float32, device="cuda")
+    with B.Photons(**bench.headline_params(cfg, precision="mixed", n_streams=4)) as ph:
+        ph.set_particles(dpos, None)
+        ph.build_leaves()
+        st = ph.short_range_acc(out)
+    a = out[torch.from_numpy(tgt).cuda()].double().cpu().numpy()
+    # an fp32 output array costs half an ulp of each acceleration on top of the arithmetic
+    assert _err(a, ref) <= TOL_FP32
+    assert st["n_leaves"] == cfg.n // 32 and bool(torch.isfinite(out).all())
+
+
 def test_full_size_config4_sampled(B, oracle):
     """BASELINE config 4 (N = 256^3 clustered, MAXLEAF 32) exactly as bench.py times it (fp32, poly g,
     close pairs on, device-resident input), checked on sampled targets the oracle computes one by one."""
