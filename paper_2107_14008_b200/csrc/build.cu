@@ -25,7 +25,7 @@ void free_leaves(Ctx* c)
 // Every tree node is split at its median along the axis of largest extent of its particle bounding box; the
 // left child takes floor(size/2) particles (A13).  Two phases:
 //   A (levels 0 .. L0-1, nodes larger than ORB_CTA_MAX particles): one stable radix sort per level over the
-//     whole array on keys (node, coordinate as a 24-bit fixed-point number inside the node's bbox).  The
+//     whole array on keys (node, coordinate as a 20-bit fixed-point number inside the node's bbox).  The
 //     particles travel with the sort as float4 {x, y, z, caller index} in current order, so every pass reads
 //     and writes coalesced; the gather that applies the sorted order also reduces the children's bboxes.
 //   B (levels L0 .. depth-1): one CTA per level-L0 node finishes all remaining levels in shared memory
@@ -34,6 +34,10 @@ void free_leaves(Ctx* c)
 
 constexpr int ORB_CTA_MAX = 4096;   // particles a phase-B CTA holds in shared memory
 constexpr int ORB_CTA_THREADS = 1024;
+// Phase-A sort key = (node, coordinate quantised to this many bits inside the node's bbox).  20 bits resolve 1e-6 of
+// the node's extent — far below the particle spacing of nodes that still hold > 4096 particles — and keep the
+// keys within 32 bits (4 radix passes or fewer) down to level 12; ties are split by the stable order.
+constexpr int ORB_COORD_BITS = 20;
 
 __global__ void orb_init_kernel(long long n, const double* __restrict__ pos, float4* __restrict__ P)
 {
@@ -112,10 +116,11 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
     const int axis = widest_axis(ext);
     const float4 p = P[q];
     const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
-    // monotone map of [lo, hi] onto 24-bit integers
+    // monotone map of [lo, hi] onto ORB_COORD_BITS-bit integers
     const float u = ext[axis] > 0.f ? (x - l[axis]) / ext[axis] : 0.f;
-    const unsigned f = (unsigned)fminf(u * 16777215.0f, 16777215.0f);
-    keys[q] = (Key)(((unsigned long long)seg << 24) | f);
+    const float top = (float)((1u << ORB_COORD_BITS) - 1u);
+    const unsigned f = (unsigned)fminf(u * top, top);
+    keys[q] = (Key)(((unsigned long long)seg << ORB_COORD_BITS) | f);
     vals[q] = (uint32_t)q;
 }
 
@@ -458,7 +463,7 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         PH_WS(lo, int, WS_ORB_LO, 3LL << L0);
         PH_WS(hi, int, WS_ORB_HI, 3LL << L0);
         size_t tmp_bytes = 0;
-        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + L0, st));
+        PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, ORB_COORD_BITS + L0, st));
         {
             size_t need32 = 0;
             PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(nullptr, need32, reinterpret_cast<uint32_t*>(keys), reinterpret_cast<uint32_t*>(keys2),
@@ -472,14 +477,14 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         orb_gather_bbox_kernel<<<blocks_for(n, tb), tb, 0, st>>>(n, 0, nullptr, P_cur, nullptr, lo, hi);
         c->launches += 3;
         for (int level = 0; level < L0; ++level) {
-            if (24 + level <= 32) {
+            if (ORB_COORD_BITS + level <= 32) {
                 uint32_t* k32 = reinterpret_cast<uint32_t*>(keys);
                 uint32_t* k32b = reinterpret_cast<uint32_t*>(keys2);
                 orb_key_kernel<uint32_t><<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, k32, vals);
-                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k32, k32b, vals, vals2, (int)n, 0, 24 + level, st));
+                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k32, k32b, vals, vals2, (int)n, 0, ORB_COORD_BITS + level, st));
             } else {
                 orb_key_kernel<unsigned long long><<<blocks_for(n, tb), tb, 0, st>>>(n, level, P_cur, lo, hi, keys, vals);
-                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, 24 + level, st));
+                PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, (int)n, 0, ORB_COORD_BITS + level, st));
             }
             ++c->launches;
             const bool more = level + 1 < L0;   // the next level's boxes, reduced while the order is applied
