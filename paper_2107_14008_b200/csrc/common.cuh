@@ -28,7 +28,10 @@ __host__ __device__ inline int entry_shift_code(unsigned y)
     if (y & ENTRY_PER_PAIR) return 27;
     return (int)((y >> 16) & 3u) + 3 * (int)((y >> 18) & 3u) + 9 * (int)((y >> 20) & 3u);
 }
-constexpr int N_STAGES = 3;         // shared-memory ring depth per warp
+#ifndef PHOTONS_STAGES
+#define PHOTONS_STAGES 3
+#endif
+constexpr int N_STAGES = PHOTONS_STAGES;   // shared-memory ring depth per warp
 
 struct GTable {                 // Eq. 2 table
     int n = 0;                  // intervals over x in [0, 3]; n + 1 nodes

@@ -8,7 +8,9 @@ namespace photons {
 size_t p32_smem_bytes(Ctx* c, int T)
 {
     const int W = c->p.warps_per_leaf;
-    size_t b = (size_t)W * N_STAGES * c->p.chunk_max * 16 + (size_t)W * N_STAGES * 8 + (size_t)W * T * 32 * 3 * 8;
+    const bool mixed = c->p.precision == PHOTONS_MIXED;
+    size_t b = (size_t)W * N_STAGES * c->p.chunk_max * 16 + (size_t)W * T * 32 * 3 * 8;
+    b += mixed ? (size_t)((W * N_STAGES * 8 + 15) & ~15) + (size_t)W * N_STAGES * MAX_RUN_LEAVES * 16 : (size_t)W * N_STAGES * 8;
     if (c->p.g_mode == PHOTONS_G_TABLE) b += (size_t)(c->table.n + 1) * 8;
     return b;
 }

@@ -24,6 +24,7 @@
 
 namespace photons {
 
+constexpr int MAX_RUN_LEAVES = 16;        // chunk_max / maxleaf at most (256 / 16)
 constexpr float R2_FLOOR = 1e-24f;       // added to every r^2: self / coincident pairs give w * 0 = 0 (A7)
 constexpr float MAGIC = 12582912.0f;     // 1.5 * 2^23: float -> nearest-integer trick for the table index
 
@@ -203,8 +204,13 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     unsigned char* ring = smem_raw + (size_t)warp * N_STAGES * stage_bytes;
     unsigned char* tail = smem_raw + (size_t)W * N_STAGES * stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES;
-    double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 8);           // W x T x 32 x 3 doubles
-    float2* tab = reinterpret_cast<float2*>(tail + W * N_STAGES * 8 + (size_t)W * T * 32 * 3 * 8);
+    // MIXED: per stage, the origin of every source leaf of the staged run minus the target leaf's origin
+    // (the region exists in the MIXED kernels only; the others keep the barriers' plain size)
+    const int bars_bytes = MIXED ? ((W * N_STAGES * 8 + 15) & ~15) : W * N_STAGES * 8;
+    float4* cshift = reinterpret_cast<float4*>(tail + bars_bytes) + warp * N_STAGES * MAX_RUN_LEAVES;
+    unsigned char* tail2 = tail + bars_bytes + (MIXED ? (size_t)W * N_STAGES * MAX_RUN_LEAVES * 16 : 0);
+    double* red = reinterpret_cast<double*>(tail2);                             // W x T x 32 x 3 doubles
+    float2* tab = reinterpret_cast<float2*>(tail2 + (size_t)W * T * 32 * 3 * 8);
 
     const long long leaf = a.order[a.first + blockIdx.x];
     const long long slot0 = leaf * M;
@@ -267,6 +273,18 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
     auto issue = [&](int k, int cur_batch, int st) {
         const uint2 e = entry(k, cur_batch);
+        if (MIXED) {
+            // origin differences in fp64, rounded once (A15); computed when the copy is issued, three runs
+            // ahead of their use, so the global loads of the origins are off the critical path
+            const int nleaf = (int)((e.y & 0xffffu) >> a.log2m);
+            if (lane < nleaf) {
+                const long long jl = (long long)(e.x >> a.log2m) + lane;
+                const int sxi = (int)((e.y >> 16) & 3u) - 1, syi = (int)((e.y >> 18) & 3u) - 1, szi = (int)((e.y >> 20) & 3u) - 1;
+                cshift[st * MAX_RUN_LEAVES + lane] = make_float4((float)((a.ctr[3 * jl] + a.Ld * sxi) - cix),
+                                                                 (float)((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy),
+                                                                 (float)((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz), 0.f);
+            }
+        }
         if (lane == 0) {
             const uint32_t bytes = (e.y & 0xffffu) * 16u;
             mbar_expect_tx_u32(bars_u32 + 8u * st, bytes);
@@ -299,12 +317,9 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             float qx[T], qy[T], qz[T];
             float sax = 0.f, say = 0.f, saz = 0.f;
             if (MIXED) {
-                const long long jl = (long long)((e.x + b0) >> a.log2m);
-                const float dcx = (float)((a.ctr[3 * jl] + a.Ld * sxi) - cix);
-                const float dcy = (float)((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy);
-                const float dcz = (float)((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz);
+                const float4 dc = cshift[st * MAX_RUN_LEAVES + (b0 >> a.log2m)];
 #pragma unroll
-                for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dcx; qy[t] = ty[t] - dcy; qz[t] = tz[t] - dcz; }
+                for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dc.x; qy[t] = ty[t] - dc.y; qz[t] = tz[t] - dc.z; }
             } else {
                 // s = +1: move the target by -L (exact, it sits in the upper half of the box);
                 // s = -1: move the sources by -L per pair (exact for the same reason)
