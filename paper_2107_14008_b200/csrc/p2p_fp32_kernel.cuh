@@ -1,6 +1,6 @@
 // fp32 / mixed-precision P2P kernel (Alg. 1 + Alg. 2, the paper's SP run L206), written for sm_100a.
 //
-// Mapping (SURVEY.md §8(a) a4-a9; DESIGN.md §5):
+// Mapping (SURVEY.md §8(a) a4-a9; DESIGN.md §6):
 //   CTA            one target leaf (Alg. 1 L96); its W warps split the leaf's source list
 //   lane           T targets in registers; the warp is split into 32 T / maxleaf lane groups that take
 //                  alternate source pairs (maxleaf 16: the two half-warps take the same 16
