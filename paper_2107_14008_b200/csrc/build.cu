@@ -125,14 +125,15 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
 }
 
 // sorts every aligned window of kmax keys ascending (kmax = n2: the whole array)
-__device__ __forceinline__ void cta_bitonic_sort(unsigned long long* key, int n2, int kmax)
+template <typename Key>
+__device__ __forceinline__ void cta_bitonic_sort(Key* key, int n2, int kmax)
 {
     for (int k = 2; k <= kmax; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
             for (int t = threadIdx.x; t < (n2 >> 1); t += blockDim.x) {
                 const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // the lower index of the t-th pair
                 const int l = i | j;
-                const unsigned long long a = key[i], b = key[l];
+                const Key a = key[i], b = key[l];
                 const bool up = (i & k) == 0 || k == kmax;
                 if ((a > b) == up) { key[i] = b; key[l] = a; }
             }
@@ -179,25 +180,37 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
             }
         }
         __syncthreads();
+        // A node that holds a power of two of particles has its sub-nodes in aligned windows: they are sorted
+        // separately (fewer bitonic stages) on 32-bit keys (coordinate quantised to 20 bits inside the sub-node's
+        // bbox | local index).  Any other size: one sort of 64-bit keys (sub-node | fp32 coordinate | local index).
+        const bool windowed = size == n2;
+        unsigned* key32 = reinterpret_cast<unsigned*>(key);
         for (int e = threadIdx.x; e < n2; e += blockDim.x) {
             unsigned long long k = ~0ULL;            // padding sorts to the end
             if (e < size) {
                 const int sub = (int)seg_of(size, sl, e);
-                float ext[3];
-                for (int a = 0; a < 3; ++a) ext[a] = ord2f(bhi[3 * sub + a]) - ord2f(blo[3 * sub + a]);
+                float lo3[3], ext[3];
+                for (int a = 0; a < 3; ++a) { lo3[a] = ord2f(blo[3 * sub + a]); ext[a] = ord2f(bhi[3 * sub + a]) - lo3[a]; }
                 const int axis = widest_axis(ext);
                 const float4 p = cur[e];
                 const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
-                k = ((unsigned long long)sub << 44) | ((unsigned long long)((unsigned)f2ord(x) ^ 0x80000000u) << 12) | (unsigned)e;
+                if (windowed) {
+                    const float u = ext[axis] > 0.f ? (x - lo3[axis]) / ext[axis] : 0.f;
+                    k = ((unsigned)fminf(u * 1048575.0f, 1048575.0f) << 12) | (unsigned)e;
+                } else {
+                    k = ((unsigned long long)sub << 44) | ((unsigned long long)((unsigned)f2ord(x) ^ 0x80000000u) << 12) | (unsigned)e;
+                }
             }
-            key[e] = k;
+            if (windowed) key32[e] = (unsigned)k;
+            else key[e] = k;
         }
         __syncthreads();
-        // when the node holds a power of two of particles its sub-nodes are aligned windows: sort them separately
-        cta_bitonic_sort(key, n2, size == n2 ? (n2 >> sl) : n2);
+        if (windowed) cta_bitonic_sort(key32, n2, n2 >> sl);
+        else cta_bitonic_sort(key, n2, n2);
         // apply the order: read through the sorted local indices, then write back
         float4 tmp[ORB_CTA_MAX / ORB_CTA_THREADS];
-        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) tmp[r] = cur[(int)(key[e] & 0xfffu)];
+        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r)
+            tmp[r] = cur[windowed ? (int)(key32[e] & 0xfffu) : (int)(key[e] & 0xfffu)];
         __syncthreads();
         for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) cur[e] = tmp[r];
         __syncthreads();
