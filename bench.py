@@ -57,7 +57,7 @@ def flops_per_pair(g_mode: str, poly_degree: int = POLY_DEGREE) -> float:
 PAPER_FLOPS_PER_PAIR = 51.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the headline kernel, from the committed
 # `ncu --set full` capture (profiles/r1_p2p_fp32_poly12_ncu_full.md): config 4, MAXLEAF 32, fp32, poly.
-NCU_TRAFFIC_BYTES = {("c4_clustered_256", 32, "fp32", "poly"): 20.123856e9 + 0.671910656e9}
+NCU_TRAFFIC_BYTES = {("c4_clustered_256", 32, "fp32", "poly"): 20.127754e9 + 0.671901440e9}
 
 
 def geometry(cfg):
