@@ -107,3 +107,28 @@ def test_poly_fit_rejects_bad_arguments():
     for deg, rc in ((0, 6.0), (21, 6.0), (12, 0.0), (12, 6.5)):
         with pytest.raises(binding.PhotonsError):
             binding.poly_fit(deg, rc)
+
+
+def test_reference_arm_json_line_on_cpu(capsys):
+    """`bench.py --impl reference` (the oracle arm) needs no GPU: run it on config 1 and check the contract keys."""
+    import json
+    import bench
+    rc = bench.main(["--impl", "reference", "--config", "1", "--steps", "1", "--warmup", "0"])
+    assert rc == 0
+    line = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["unit"] == "pairs/s" and line["higher_is_better"] is True
+    assert line["n_gpus"] == 1 and line["steps"] == 1 and line["warmup"] == 0 and line["vs_baseline"] is None
+    assert line["value"] > 0 and line["ms_per_step"] > 0 and line["dtype"] == "f64" and line["data"] == "synthetic"
+    assert line["config"]["workload"] == "c1_uniform_32"
+    cb = line["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] == line["value"] and "targets" in cb["sample"]
+    assert line["e2e"] == {"value": line["value"], "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    # all 32^3 targets against all sources: 2^30 pair tests, 1563.5 neighbours per particle on average
+    assert cb["within_cut_pairs_per_s"] / cb["value"] == pytest.approx(1563.5 / 32768, rel=0.01)
+
+
+def test_reference_arm_is_silent_on_other_ranks(capsys, monkeypatch):
+    import bench
+    monkeypatch.setenv("RANK", "1")
+    assert bench.main(["--impl", "reference", "--config", "1", "--steps", "1", "--warmup", "0"]) == 0
+    assert capsys.readouterr().out.strip() == ""
