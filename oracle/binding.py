@@ -42,7 +42,7 @@ def _load():
         lib.oracle_p2p.argtypes = [
             ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
             ctypes.c_longlong, ctypes.c_void_p,
-            ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+            ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double,
             ctypes.c_void_p, ctypes.c_void_p]
         _lib = lib
     return _lib
@@ -60,7 +60,7 @@ def oracle_T(x):
     return out if np.ndim(x) else float(out[0])
 
 
-def _call(pos, mass, tgt, boxsize, r_s, r_cut, G):
+def _call(pos, mass, tgt, boxsize, r_s, r_cut, G, eps=0.0):
     lib = _load()
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     n = pos.shape[0]
@@ -76,16 +76,17 @@ def _call(pos, mass, tgt, boxsize, r_s, r_cut, G):
     counts = np.zeros(2, dtype=np.int64)
     if nt:
         lib.oracle_p2p(n, pos.ctypes.data, mass.ctypes.data, nt, tptr,
-                       float(boxsize), float(r_s), float(r_cut), float(G),
+                       float(boxsize), float(r_s), float(r_cut), float(G), float(eps),
                        acc.ctypes.data, counts.ctypes.data)
     return acc, {"pair_tests": int(counts[0]), "pairs_in_cut": int(counts[1])}
 
 
-def p2p(pos, mass, *, boxsize, r_s, r_cut, G=1.0):
-    """Full O(N^2) sum: acc[n,3] and counters.  boxsize <= 0 means isolated boundaries (no images)."""
-    return _call(pos, mass, None, boxsize, r_s, r_cut, G)
+def p2p(pos, mass, *, boxsize, r_s, r_cut, G=1.0, eps=0.0):
+    """Full O(N^2) sum: acc[n,3] and counters.  boxsize <= 0 means isolated boundaries (no images);
+    eps > 0 = Plummer softening length (A23)."""
+    return _call(pos, mass, None, boxsize, r_s, r_cut, G, eps)
 
 
-def p2p_sampled(pos, mass, targets, *, boxsize, r_s, r_cut, G=1.0):
+def p2p_sampled(pos, mass, targets, *, boxsize, r_s, r_cut, G=1.0, eps=0.0):
     """Accelerations of the listed targets against all N sources."""
-    return _call(pos, mass, targets, boxsize, r_s, r_cut, G)
+    return _call(pos, mass, targets, boxsize, r_s, r_cut, G, eps)

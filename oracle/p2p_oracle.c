@@ -14,6 +14,11 @@
  *         L55 "F_s = -r/r^3 T" with r = r_i - r_j; A3)
  *   pairs with r == 0 (self, coincident) contribute nothing                  (A7)
  *   pairs with r >= r_cut contribute nothing                                 (north_star; A8)
+ *   softening ("100 h^-1 kpc softening length"; form not given; A23): with eps > 0
+ *          the short-range potential psi(r) = erfc(r/2r_s)/r is taken at r_eps = sqrt(r^2 + eps^2)
+ *          (Plummer substitution), whose gradient gives
+ *              a_i = G * sum_{j: 0 < |d_ij|, r_eps < r_cut}  m_j * d_ij * T(r_eps; r_s) / r_eps^3 ;
+ *          eps = 0 is the unsoftened sum above, bit for bit.
  *
  * The leaf structure, MAXLEAF and the interaction-list criterion do not enter: a pair outside
  * r_cut contributes exactly zero, so the sum over listed leaves equals this all-pairs sum
@@ -54,13 +59,15 @@ int oracle_num_threads(void)
  * pos: n x 3 row-major doubles, mass: n doubles, acc: nt x 3 doubles (output).
  * counts (may be NULL): counts[0] += pair tests done, counts[1] += pairs inside r_cut.
  * tgt == NULL means targets 0..nt-1 (nt == n gives the full O(N^2) sum).
+ * eps: Plummer softening length (A23), 0 = none.
  */
 void oracle_p2p(long long n, const double *pos, const double *mass,
                 long long nt, const long long *tgt,
-                double L, double r_s, double r_cut, double G,
+                double L, double r_s, double r_cut, double G, double eps,
                 double *acc, long long *counts)
 {
     const double rcut2 = r_cut * r_cut;
+    const double eps2 = eps * eps;                     /* A23; 0 = no softening */
     const double inv2rs = 1.0 / (2.0 * r_s);
     long long n_tests = 0, n_in = 0;
 
@@ -80,9 +87,10 @@ void oracle_p2p(long long n, const double *pos, const double *mass,
                 dz -= L * nearbyint(dz / L);
             }
             const double r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 > 0.0 && r2 < rcut2) {
-                const double r = sqrt(r2);
-                const double grav = G * mass[j] * oracle_T(r * inv2rs) / (r2 * r);
+            const double r2e = r2 + eps2;              /* r_eps^2; == r2 when eps == 0 */
+            if (r2 > 0.0 && r2e < rcut2) {
+                const double r = sqrt(r2e);
+                const double grav = G * mass[j] * oracle_T(r * inv2rs) / (r2e * r);
                 ax += (long double)(grav * dx);
                 ay += (long double)(grav * dy);
                 az += (long double)(grav * dz);

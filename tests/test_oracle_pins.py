@@ -361,3 +361,103 @@ def test_isolated_equals_periodic_far_from_the_faces(oracle):
     # and Newton's third law holds in the isolated mode too
     tot = (mass[:, None] * iso).sum(axis=0)
     assert np.abs(tot).max() <= 1e-12 * (mass[:, None] * np.abs(iso)).sum()
+
+
+# ---------------------------------------- Plummer softening (reading A23)
+
+def _psi_mp(r, r_s):
+    """Short-range potential of a unit mass, psi(r) = erfc(r/2r_s)/r (D_n = grad^n psi)."""
+    return mpmath.erfc(r / (2 * r_s)) / r
+
+
+def test_softening_zero_is_the_unsoftened_sum_bitwise(oracle, small_uniform):
+    cfg, pos, mass, r_s = small_uniform
+    kw = dict(boxsize=1.0, r_s=r_s, r_cut=6 * r_s)
+    a0, c0 = oracle.p2p(pos, mass, **kw)
+    a1, c1 = oracle.p2p(pos, mass, eps=0.0, **kw)
+    a2, c2 = oracle.p2p(pos, mass, eps=1e-200, **kw)        # eps^2 underflows to 0
+    assert np.array_equal(a0, a1) and np.array_equal(a0, a2) and c0 == c1 == c2
+    # and a softening far below every pair separation changes the sum only at round-off level
+    a3, _ = oracle.p2p(pos, mass, eps=1e-9, **kw)
+    rms = np.sqrt((a0 ** 2).sum(axis=1).mean())
+    assert np.abs(a3 - a0).max() < 1e-9 * rms
+
+
+@pytest.mark.parametrize("eps_over_d", [0.01, 0.5, 1.0, 3.0, 40.0])
+def test_softened_two_body_is_minus_gradient_of_plummer_substituted_potential(oracle, eps_over_d):
+    """A23: a_1 = -grad_1 [ -G m_2 psi( sqrt(|r_1 - r_2|^2 + eps^2) ) ], by 40-digit numerical differentiation —
+    fixes the direction vector (the unsoftened d), the radius in T and in 1/r^3 (both r_eps) and the sign."""
+    n_pm, G = 32, 1.7
+    r_s = 1.2 / n_pm
+    dvec = np.array([0.004, -0.003, 0.0012])
+    eps = eps_over_d * float(np.linalg.norm(dvec))
+    if np.hypot(np.linalg.norm(dvec), eps) >= 6 * r_s:
+        pytest.skip("beyond the cut")
+    p1 = np.array([0.31, 0.52, 0.77])
+    pos = np.array([p1, p1 + dvec])
+    mass = np.array([0.4, 0.9])
+    acc, cnt = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=6 * r_s, G=G, eps=eps)
+    assert cnt["pairs_in_cut"] == 2
+    with mpmath.workdps(40):
+        def phi(x, y, z):      # potential at particle 1's position due to particle 2
+            d2 = (pos[1, 0] - x) ** 2 + (pos[1, 1] - y) ** 2 + (pos[1, 2] - z) ** 2
+            return -G * mass[1] * _psi_mp(mpmath.sqrt(d2 + mpmath.mpf(eps) ** 2), mpmath.mpf(r_s))
+        want = [-mpmath.diff(phi, tuple(p1), tuple(int(k == a) for k in range(3))) for a in range(3)]
+    assert acc[0] == pytest.approx([float(v) for v in want], rel=1e-11)
+    assert 0.4 * acc[0] + 0.9 * acc[1] == pytest.approx([0, 0, 0], abs=1e-13 * np.abs(acc).max())
+
+
+def test_softened_closed_form_limits_and_cut(oracle):
+    n_pm = 32
+    r_s = 1.2 / n_pm
+    r_cut = 6 * r_s
+    d, eps = 0.01, 0.02
+    pos = np.array([[0.5, 0.5, 0.5], [0.5 + d, 0.5, 0.5]])
+    mass = np.array([1.0, 2.0])
+    acc, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=eps)
+    re = math.hypot(d, eps)
+    assert acc[0, 0] == pytest.approx(2.0 * float(T_mp(re / (2 * r_s))) * d / re ** 3, rel=1e-13)
+    # deep inside the softening core the force is linear in d: a -> G m d T(eps)/eps^3
+    tiny = 1e-7
+    pos[1, 0] = 0.5 + tiny
+    acc, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=eps)
+    assert acc[0, 0] == pytest.approx(2.0 * float(T_mp(eps / (2 * r_s))) * tiny / eps ** 3, rel=1e-9)
+    # coincident particles still contribute nothing (d = 0), and the cut acts on r_eps: a pair with
+    # r < r_cut <= r_eps is outside
+    pos[1] = pos[0]
+    acc, cnt = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=eps)
+    assert np.all(acc == 0.0) and cnt["pairs_in_cut"] == 0
+    pos[1] = pos[0] + [0.99 * r_cut, 0, 0]
+    a_in, c_in = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=0.1 * r_cut)
+    a_out, c_out = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=0.2 * r_cut)
+    assert c_in["pairs_in_cut"] == 2 and c_out["pairs_in_cut"] == 0 and np.all(a_out == 0.0)
+
+
+def test_softened_third_law_and_brute_force(oracle):
+    rng = np.random.default_rng(321)
+    n, n_pm = 48, 16
+    r_s = 1.2 / n_pm
+    r_cut = 6 * r_s
+    eps = 0.03
+    pos = np.mod(rng.random((n, 3)) * 0.5 + 0.8, 1.0)      # straddles the seam
+    mass = rng.uniform(0.5, 1.5, n)
+    acc, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=eps)
+    tot = (mass[:, None] * acc).sum(axis=0)
+    assert np.abs(tot).max() <= 1e-12 * (mass[:, None] * np.abs(acc)).sum()
+    with mpmath.workdps(30):
+        ref = np.zeros((n, 3))
+        for i in range(n):
+            a = [mpmath.mpf(0)] * 3
+            for j in range(n):
+                d = [mpmath.mpf(pos[j, k]) - mpmath.mpf(pos[i, k]) for k in range(3)]
+                d = [dk - mpmath.nint(dk) for dk in d]
+                r2 = sum(dk * dk for dk in d)
+                r2e = r2 + mpmath.mpf(eps) ** 2
+                if r2 > 0 and r2e < mpmath.mpf(r_cut) ** 2:
+                    re = mpmath.sqrt(r2e)
+                    x = re / (2 * mpmath.mpf(r_s))
+                    T = mpmath.erfc(x) + 2 * x / mpmath.sqrt(mpmath.pi) * mpmath.exp(-x * x)
+                    w = mpmath.mpf(mass[j]) * T / re ** 3
+                    a = [a[k] + w * d[k] for k in range(3)]
+            ref[i] = [float(v) for v in a]
+    assert np.abs(acc - ref).max() <= 1e-14 * np.abs(ref).max()
