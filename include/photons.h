@@ -39,8 +39,9 @@ enum {
     PHOTONS_ENOMEM = 3,     /* host or device allocation failed */
     PHOTONS_ECUDA = 4,      /* CUDA runtime error (message in photons_last_error) */
     PHOTONS_ENODEVICE = 5,  /* no usable CUDA device */
-    PHOTONS_EBOX = 6,       /* r_cut >= boxsize/2, or 2 r_cut + leaf extents >= boxsize (minimum image
-                               per list entry would be ambiguous; A10) */
+    PHOTONS_EBOX = 6,       /* periodic box with r_cut >= boxsize/2: the minimum image is not unique (photons_create).
+                               Leaves so large that 2 r_cut + both extents >= boxsize are NOT an error: their list
+                               entries take the minimum image per pair instead (shift code 27; A10) */
     PHOTONS_ENONFINITE = 7  /* NaN/Inf in positions or masses */
 };
 
@@ -60,6 +61,13 @@ enum {
                              s = (r/2r_s)^2 and Q an FMA-pipe polynomial (fp32 paths only) */
 };
 
+/* what the interpolation table holds per node (PHOTONS_G_TABLE) */
+enum {
+    PHOTONS_TABLE_PAPER = 0, /* {T_i, E_i} as in the paper (L143); the polynomials of Eq. 2 in x_i are rebuilt per pair */
+    PHOTONS_TABLE_COEF = 1   /* the Taylor coefficients of Eq. 2 themselves, T^(k)(x_i) h^k / k!, k = 0..table_level: the
+                                same series about the same node, Horner only (PHOTONS_FP64 only) */
+};
+
 enum { PHOTONS_MEM_HOST = 0, PHOTONS_MEM_DEVICE = 1 };
 
 /* element type of caller arrays (pos, mass, acc) */
@@ -76,7 +84,8 @@ typedef struct {
     int precision;            /* PHOTONS_FP64 / FP32 / MIXED */
     int g_mode;               /* PHOTONS_G_* */
     int table_nodes;          /* TABLE: number of intervals n over x in [0,3] (n+1 nodes), 64..4096; paper: 512 */
-    int table_level;          /* TABLE: highest Taylor term kept, 0..4 (paper: T[2] for SP, T[4] for DP, L149) */
+    int table_level;          /* TABLE: highest Taylor term kept (paper: T[2] for SP, T[4] for DP, L149): 0..4 with
+                                 PHOTONS_FP64, 0..3 with FP32 / MIXED (T[2] already sits on the fp32 floor) */
     int n_streams;            /* >= 1: target-leaf batches are issued round-robin over this many CUDA streams */
     int device;               /* CUDA device ordinal */
     double close_pair_radius; /* fp32/mixed paths: pairs with 0 < r < this are evaluated in fp64 inside the
@@ -92,6 +101,10 @@ typedef struct {
     int periodic;             /* 1 = periodic cube of side boxsize, minimum image (default; north_star);
                                  0 = isolated boundaries: no images, positions are not wrapped,
                                  boxsize only sets r_s = rs_over_cell * boxsize / n_pm */
+    double softening;         /* Plummer softening length eps >= 0 (A23): the pair function is
+                                 taken at r_eps = sqrt(r^2 + eps^2), a_i += G m_j d_ij g(r_eps) / r_eps^3 for pairs with
+                                 0 < r and r_eps < r_cut.  0 = none (default; north_star's formula) */
+    int table_layout;         /* TABLE: PHOTONS_TABLE_PAPER (default) or PHOTONS_TABLE_COEF */
 } photons_params;
 
 typedef struct {
@@ -109,7 +122,7 @@ typedef struct {
 } photons_stats;
 
 /* Fill *p with the paper's defaults: boxsize 1, n_pm 32, rs_over_cell 1.2, rcut_over_rs 6, G 1, maxleaf 32,
- * FP32, G_POLY, table 512/level 2, 1 stream, device 0, close pairs off, chunk_max default, periodic. */
+ * FP32, G_POLY, table 512/level 2, 1 stream, device 0, close pairs off, chunk_max default, periodic, no softening. */
 void photons_default_params(photons_params* p);
 
 /* Validate parameters, select the device, create streams, build the g table (TABLE mode; fp64 on the
@@ -125,7 +138,9 @@ int photons_set_stream(photons_ctx* ctx, void* cuda_stream);
 
 /* Copy n particles in.  pos: n x 3 row-major, mass: n values or NULL (= 1/n each), both of element type
  * dtype (PHOTONS_DTYPE_*), both host or both device memory as tagged.  Positions are wrapped into
- * [0, boxsize).  cuda_stream: a cudaStream_t the device-side copy is enqueued on (NULL = the context's main stream);
+ * [0, boxsize).  Any units: the fp32 / mixed kernels work on positions divided by a power of two near r_cut and
+ * on G m_j divided by a power of two >= max |G m_j| (both exact rescalings, undone in fp64 on output), so
+ * neither a large G m nor a large or tiny boxsize can overflow or underflow their fp32 arithmetic.  cuda_stream: a cudaStream_t the device-side copy is enqueued on (NULL = the context's main stream);
  * the call returns after the copy has completed.  Errors: EINVAL (n < 1, or more than 2^31 - 1 particle slots),
  * ENONFINITE, ENOMEM, ECUDA. */
 int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const void* mass, int dtype,
@@ -154,15 +169,14 @@ int photons_get_interaction_list(photons_ctx* ctx, long long* chunk_ptr, int* fi
 /* Statistics of the last build / run. */
 int photons_get_stats(photons_ctx* ctx, photons_stats* stats);
 
-/* Device throughput micro-benchmarks that give the roofline denominators:
- * kind 0 = FFMA (register operands), 1 = FFMA2 (fma.rn.f32x2), 2 = DFMA, 3 = MUFU.RSQ,
- * 4 = FFMA2 with 2 MUFU.RSQ per 8 (FFMA2 lanes counted), 5 = LDS.128 broadcast, 6 = FFMA with immediates,
- * 7 = FFMA2 with 4 ALU-pipe ops per 8 (FFMA2 lanes counted), 8 = FADD2, 9 = FMUL2, 10 = FFMA2 without
- * operand reuse; 11..15 = the pair core's mix per step, 24 FFMA2 in two dependent chains (14) plus 2 MUFU.RSQ (11),
- * plus 2 FSETP+FSEL (12), or plus 2 broadcast LDS.128 (13), or plus both (15); 16 / 17 = kind 10 plus 4 / 8 integer
- * ALU ops per 8 FFMA2 — FFMA2 lanes counted.
- * kind + 100 b (b = 1..7) runs the probe with only b resident blocks of 8 warps per SM.  *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction
- * counts 2 per lane; multiply FMA rates by 2 for flops).  Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
+/* Device throughput micro-benchmarks: the measured roofline denominators next to the nominal
+ * SM-count x lanes x clock figure.  kind 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2), 2 = DFMA, 3 = MUFU.RSQ, 4 = MUFU.EX2,
+ * 5 = LDS.128 broadcast, 6 = DADD, 7 = MUFU.RSQ64H, 8 = FADD2, 9 = FMUL2;
+ * 11..15 = ceiling of the fp32 pair core's own instruction mix per step (two pairs per lane): 24 FFMA2 in two dependent
+ * chains (14), plus 2 MUFU.RSQ (11), plus 2 FSETP+FSEL (12), or plus 2 broadcast LDS.128 (13), or plus both (15).
+ * kind + 100 b (b = 1..7) runs the probe with only b resident blocks of 8 warps per SM.
+ * *out = lane-operations per second summed over the chip (one FMA = 1; an f32x2 instruction counts 2 per lane;
+ * multiply FMA rates by 2 for flops).  Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
 int photons_peak_probe(int device, int kind, double* out);
 
 /* Host-only (needs no device): the polynomial behind PHOTONS_G_POLY.  With s = (r/2r_s)^2, s_max = (rcut_over_rs/2)^2

@@ -17,11 +17,13 @@ LIB_PATH = os.path.join(_HERE, "libphotons.so")
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENODEVICE, EBOX, ENONFINITE = range(8)
 FP64, FP32, MIXED = 0, 1, 2
 G_DIRECT, G_TABLE, G_POLY = 0, 1, 2
+TABLE_PAPER, TABLE_COEF = 0, 1
 MEM_HOST, MEM_DEVICE = 0, 1
 DTYPE_F64, DTYPE_F32 = 0, 1
 
 PRECISIONS = {"fp64": FP64, "fp32": FP32, "mixed": MIXED}
 G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY}
+TABLE_LAYOUTS = {"paper": TABLE_PAPER, "coef": TABLE_COEF}
 ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX", "ENONFINITE"]
 
 EXPORTS = [
@@ -39,6 +41,7 @@ class Params(ctypes.Structure):
         ("table_level", ctypes.c_int), ("n_streams", ctypes.c_int), ("device", ctypes.c_int),
         ("close_pair_radius", ctypes.c_double), ("chunk_max", ctypes.c_int), ("warps_per_leaf", ctypes.c_int),
         ("targets_per_lane", ctypes.c_int), ("poly_degree", ctypes.c_int), ("periodic", ctypes.c_int),
+        ("softening", ctypes.c_double), ("table_layout", ctypes.c_int),
     ]
 
 
@@ -111,6 +114,8 @@ def default_params(**overrides) -> Params:
             v = PRECISIONS[v]
         if k == "g_mode" and isinstance(v, str):
             v = G_MODES[v]
+        if k == "table_layout" and isinstance(v, str):
+            v = TABLE_LAYOUTS[v]
         if not hasattr(p, k):
             raise TypeError(f"unknown parameter {k!r}")
         setattr(p, k, v)

@@ -21,6 +21,15 @@ int fail(Ctx* c, int code, const char* fmt, ...)
     return code;
 }
 
+cudaError_t opt_in_smem(Ctx* c, const void* kernel, size_t bytes)
+{
+    for (const void* k : c->smem_opted)
+        if (k == kernel) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) c->smem_opted.push_back(kernel);
+    return e;
+}
+
 void* workspace(Ctx* c, int slot, size_t bytes)
 {
     DevBuf& b = c->ws[slot];
@@ -53,14 +62,16 @@ static double now_ms()
     return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
 }
 
-// wrap into [0, L), flag non-finite values; src is fp64 or fp32
+// wrap into [0, L), flag non-finite values, find max |m| (the fp32 kernels' mass unit); src is fp64 or fp32.
+// flags: [0] = non-finite input seen, [1] = bits of max |m| (non-negative doubles order like their bit patterns)
 template <typename Tin>
 __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Tin* __restrict__ mass, double L, int periodic,
                               double default_mass, double* __restrict__ opos, double* __restrict__ omass,
-                              int* __restrict__ bad)
+                              unsigned long long* __restrict__ flags)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const bool live = i < n;
+    if (!live) i = n - 1;
     bool ok = true;
     for (int a = 0; a < 3; ++a) {
         double x = (double)pos[3 * i + a];
@@ -70,19 +81,15 @@ __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Ti
             if (x >= L) x -= L;      // x/L rounding can leave x == L
             if (x < 0.0) x = 0.0;
         }
-        opos[3 * i + a] = x;
+        if (live) opos[3 * i + a] = x;
     }
     double m = mass ? (double)mass[i] : default_mass;
     if (!isfinite(m)) { ok = false; m = 0.0; }
-    omass[i] = m;
-    if (!ok) atomicExch(bad, 1);
-}
-
-template <typename Tout>
-__global__ void convert_out_kernel(long long n3, const double* __restrict__ in, Tout* __restrict__ out)
-{
-    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i < n3) out[i] = (Tout)in[i];
+    if (live) omass[i] = m;
+    if (!ok) atomicExch(&flags[0], 1ULL);
+    unsigned long long mb = (unsigned long long)__double_as_longlong(fabs(m));
+    for (int o = 16; o > 0; o >>= 1) mb = max(mb, __shfl_xor_sync(0xffffffffu, mb, o));
+    if ((threadIdx.x & 31) == 0 && mb > 0) atomicMax(&flags[1], mb);
 }
 
 static void free_particles(Ctx* c)
@@ -120,6 +127,8 @@ void photons_default_params(photons_params* p)
     p->targets_per_lane = 0;
     p->poly_degree = 0;
     p->periodic = 1;
+    p->softening = 0.0;
+    p->table_layout = PHOTONS_TABLE_PAPER;
 }
 
 static int create_fail(char* err_buf, int err_len, int code, const char* msg)
@@ -147,6 +156,12 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.g_mode == PHOTONS_G_TABLE) {
         if (p.table_nodes < 64 || p.table_nodes > 4096) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_nodes must be 64..4096");
         if (p.table_level < 0 || p.table_level > 4) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_level must be 0..4");
+        if (p.table_level > 3 && p.precision != PHOTONS_FP64)
+            return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_level 4 needs PHOTONS_FP64 (the fp32 kernels keep T[0..3])");
+        if (p.table_layout != PHOTONS_TABLE_PAPER && p.table_layout != PHOTONS_TABLE_COEF)
+            return create_fail(err_buf, err_len, PHOTONS_EINVAL, "bad table_layout");
+        if (p.table_layout == PHOTONS_TABLE_COEF && p.precision != PHOTONS_FP64)
+            return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF is an option of the PHOTONS_FP64 path");
     }
     if (p.n_streams < 1 || p.n_streams > 64) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "n_streams must be 1..64");
     if (p.close_pair_radius < 0 || !std::isfinite(p.close_pair_radius)) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be >= 0");
@@ -170,6 +185,8 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.periodic != 0 && p.periodic != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "periodic must be 0 or 1");
     if (p.periodic && !(r_cut < 0.5 * p.boxsize)) return create_fail(err_buf, err_len, PHOTONS_EBOX, "r_cut >= boxsize/2: minimum image is not unique");
     if (p.close_pair_radius >= r_cut) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be < r_cut");
+    if (!(p.softening >= 0) || !std::isfinite(p.softening) || p.softening >= r_cut)
+        return create_fail(err_buf, err_len, PHOTONS_EINVAL, "softening must be >= 0 and < r_cut");
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -189,6 +206,8 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     c->p = p;
     c->r_s = r_s;
     c->r_cut = r_cut;
+    // length unit of the fp32 kernels: the power of two just below r_cut (an exact rescaling of fp32 data)
+    c->pscale = std::ldexp(1.0, (int)std::floor(std::log2(r_cut)));
     c->sm_count = prop.multiProcessorCount;
     bool ok = true;
     c->streams.resize(p.n_streams);
@@ -237,8 +256,8 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     const size_t esz = dtype == PHOTONS_DTYPE_F64 ? 8 : 4;
     c->d_pos = static_cast<double*>(workspace(c, WS_POS, sizeof(double) * 3 * n));
     c->d_mass = static_cast<double*>(workspace(c, WS_MASS, sizeof(double) * n));
-    int* d_bad = static_cast<int*>(workspace(c, WS_FLAG, sizeof(int)));
-    if (!c->d_pos || !c->d_mass || !d_bad) { free_particles(c); return PHOTONS_ENOMEM; }
+    unsigned long long* d_flags = static_cast<unsigned long long*>(workspace(c, WS_FLAG, 2 * sizeof(unsigned long long)));
+    if (!c->d_pos || !c->d_mass || !d_flags) { free_particles(c); return PHOTONS_ENOMEM; }
     const void *src_pos = pos, *src_mass = mass;
     if (mem_kind == PHOTONS_MEM_HOST) {
         void* d_in_pos = workspace(c, WS_IN_POS, esz * 3 * n);
@@ -252,19 +271,24 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
             src_mass = d_in_mass;
         }
     }
-    PH_CUDA(c, cudaMemsetAsync(d_bad, 0, sizeof(int), st));
+    PH_CUDA(c, cudaMemsetAsync(d_flags, 0, 2 * sizeof(unsigned long long), st));
     const int tb = 256;
     const unsigned nb = (unsigned)((n + tb - 1) / tb);
     if (dtype == PHOTONS_DTYPE_F64)
-        intake_kernel<double><<<nb, tb, 0, st>>>(n, (const double*)src_pos, (const double*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
+        intake_kernel<double><<<nb, tb, 0, st>>>(n, (const double*)src_pos, (const double*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_flags);
     else
-        intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_bad);
+        intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_flags);
     ++c->launches;
-    int bad = 0;
-    cudaError_t e = cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+    unsigned long long h_flags[2] = {0, 0};
+    cudaError_t e = cudaMemcpyAsync(h_flags, d_flags, sizeof h_flags, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { free_particles(c); return fail(c, PHOTONS_ECUDA, "set_particles: %s", cudaGetErrorString(e)); }
-    if (bad) { free_particles(c); return fail(c, PHOTONS_ENONFINITE, "set_particles: NaN or Inf in positions or masses"); }
+    if (h_flags[0]) { free_particles(c); return fail(c, PHOTONS_ENONFINITE, "set_particles: NaN or Inf in positions or masses"); }
+    // mass unit of the fp32 kernels: the power of two >= max |G m| (exact rescaling; G m / unit in (1/2, 1])
+    double m_max;
+    memcpy(&m_max, &h_flags[1], sizeof m_max);
+    const double gm_max = std::fabs(c->p.G) * m_max;
+    c->gmscale = gm_max > 0 && std::isfinite(gm_max) ? std::ldexp(1.0, (int)std::ceil(std::log2(gm_max))) : 1.0;
     c->n = n;
     return PHOTONS_OK;
 }
@@ -398,6 +422,7 @@ void photons_destroy(photons_ctx* ctx)
     workspace_free(c);
     cudaFree(c->table.d_TE);
     cudaFree(c->table.d_TE64);
+    cudaFree(c->table.d_C64);
     if (!c->streams.empty()) c->streams[0] = c->own_stream0;
     for (auto s : c->streams) if (s) cudaStreamDestroy(s);
     for (auto e : c->stream_done) if (e) cudaEventDestroy(e);

@@ -251,6 +251,7 @@ __global__ void leaf_table_kernel(long long n, int depth, long long n_leaves, co
 // one thread per slot: fill the packed arrays.  Padding slots repeat the leaf's first particle with
 // zero mass (they add nothing as sources and are never written as targets).
 __global__ void pack_kernel(long long n, int depth, int maxleaf, long long n_slots, double G, int precision,
+                            double inv_pscale, double inv_gmscale,
                             const uint32_t* __restrict__ perm, const double* __restrict__ pos,
                             const double* __restrict__ mass, const double* __restrict__ ctr,
                             int* __restrict__ slot_src, double4* __restrict__ p64, float* __restrict__ p32)
@@ -272,10 +273,11 @@ __global__ void pack_kernel(long long n, int depth, int maxleaf, long long n_slo
         double ox = 0, oy = 0, oz = 0;
         if (precision == PHOTONS_MIXED) { ox = ctr[3 * k]; oy = ctr[3 * k + 1]; oz = ctr[3 * k + 2]; }
         float* b = p32 + (s >> 1) * 8 + (s & 1);
-        b[0] = (float)(x - ox);
-        b[2] = (float)(y - oy);
-        b[4] = (float)(z - oz);
-        b[6] = (float)gm;
+        // kernel units (powers of two: the rescaling itself is exact)
+        b[0] = (float)((x - ox) * inv_pscale);
+        b[2] = (float)((y - oy) * inv_pscale);
+        b[4] = (float)((z - oz) * inv_pscale);
+        b[6] = (float)(gm * inv_gmscale);
     }
 }
 
@@ -558,7 +560,8 @@ int build_leaves_impl(Ctx* c)
         double* leaf_lo = c->d_node_lo + 3 * (n_leaves - 1);
         double* leaf_hi = c->d_node_hi + 3 * (n_leaves - 1);
         leaf_table_kernel<<<blocks_for(n_leaves, 128), 128, 0, st>>>(n, depth, n_leaves, c->d_perm, c->d_pos, c->d_leaf_cnt, leaf_lo, leaf_hi, c->d_leaf_ctr);
-        pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, c->d_perm, c->d_pos, c->d_mass,
+        pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, 1.0 / c->pscale, 1.0 / c->gmscale,
+                                                            c->d_perm, c->d_pos, c->d_mass,
                                                             c->d_leaf_ctr, c->d_slot_src, c->d_p64, c->d_p32);
         c->launches += 2;
         for (int level = depth - 1; level >= 0; --level) {

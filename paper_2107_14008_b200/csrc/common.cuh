@@ -38,6 +38,7 @@ struct GTable {                 // Eq. 2 table
     int level = 2;
     float2* d_TE = nullptr;     // {T_i, E_i} per node (fp32)
     double2* d_TE64 = nullptr;  // fp64 copy for the fp64 path
+    double* d_C64 = nullptr;    // coefficient layout (PHOTONS_TABLE_COEF): 5 doubles per node, T^(k)(x_i) h^k / k!
 };
 
 constexpr int POLY_MAX_DEG = 20;
@@ -56,7 +57,12 @@ struct DevBuf { void* p = nullptr; size_t cap = 0; };
 struct Ctx {
     photons_params p{};
     double r_s = 0, r_cut = 0;
+    // units of the fp32 / mixed kernels (powers of two, so that rescaling fp32 data is exact): lengths are divided by
+    // pscale (the power of two just below r_cut), G m by gmscale (the power of two >= max |G m|); sums are scaled back
+    // in fp64 by gmscale / pscale^2 when they are stored
+    double pscale = 1.0, gmscale = 1.0;
     int sm_count = 0;
+    std::vector<const void*> smem_opted;  // kernels whose dynamic shared-memory limit has been raised already
     std::vector<cudaStream_t> streams;   // [0] = main stream (the caller's after photons_set_stream)
     cudaStream_t own_stream0 = nullptr;  // the stream created for slot 0 (destroyed with the context)
     long long launches = 0;              // kernels of this library launched so far (cub's are not counted)
@@ -102,6 +108,8 @@ void* workspace(Ctx* c, int slot, size_t bytes);
 void workspace_free(Ctx* c);
 
 int fail(Ctx* c, int code, const char* fmt, ...);
+// raise a kernel's dynamic shared-memory limit once per context (the size per kernel is fixed by the parameters)
+cudaError_t opt_in_smem(Ctx* c, const void* kernel, size_t bytes);
 #define PH_CUDA(c, call)                                                                         \
     do {                                                                                         \
         cudaError_t e_ = (call);                                                                 \

@@ -19,12 +19,20 @@ int make_table(Ctx* c)
     const int n = c->p.table_nodes;
     std::vector<float2> te(n + 1);
     std::vector<double2> te64(n + 1);
+    std::vector<double> c64((size_t)(n + 1) * 5);
+    const long double h = 3.0L / n;
     for (int i = 0; i <= n; ++i) {
         const long double x = 3.0L * i / n;                                  // nodes over x in [0, 3] (L143)
         const long double E = -4.0L * expl(-x * x) / sqrtl(PI_L);            // E_i = -4 exp(-x_i^2)/sqrt(pi)
         const long double T = erfcl(x) - x * E / 2.0L;                       // T_i = erfc(x_i) - x_i E_i / 2
         te[i] = make_float2((float)T, (float)E);
         te64[i] = make_double2((double)T, (double)E);
+        // coefficient layout: the terms T[k] of Eq. 2 (L129-L141) with eps = e_u h, e_u in node units
+        const long double x2 = x * x;
+        const long double ck[5] = {T, x2 * E, -x * (x2 - 1.0L) * E, (2.0L / 3.0L * x2 * x2 - 5.0L / 3.0L * x2 + 1.0L / 3.0L) * E,
+                                   -x * (x2 * x2 / 3.0L - 1.5L * x2 + 1.0L) * E};
+        long double hk = 1.0L;
+        for (int k = 0; k < 5; ++k) { c64[(size_t)i * 5 + k] = (double)(ck[k] * hk); hk *= h; }
     }
     c->table.n = n;
     c->table.level = c->p.table_level;
@@ -32,6 +40,8 @@ int make_table(Ctx* c)
     PH_CUDA(c, cudaMemcpy(c->table.d_TE, te.data(), sizeof(float2) * (n + 1), cudaMemcpyHostToDevice));
     PH_CUDA(c, cudaMalloc(&c->table.d_TE64, sizeof(double2) * (n + 1)));
     PH_CUDA(c, cudaMemcpy(c->table.d_TE64, te64.data(), sizeof(double2) * (n + 1), cudaMemcpyHostToDevice));
+    PH_CUDA(c, cudaMalloc(&c->table.d_C64, sizeof(double) * c64.size()));
+    PH_CUDA(c, cudaMemcpy(c->table.d_C64, c64.data(), sizeof(double) * c64.size(), cudaMemcpyHostToDevice));
     return PHOTONS_OK;
 }
 
@@ -164,8 +174,10 @@ int make_poly(Ctx* c)
     const int deg = c->p.poly_degree;
     std::vector<long double> mono;
     c->poly_err = (double)fit_poly(deg, c->p.rcut_over_rs, mono);
-    // scale by (1/2r_s)^3 and round once; Horner order (highest degree first)
-    const long double k3 = 1.0L / (8.0L * (long double)c->r_s * c->r_s * c->r_s);
+    // scale by (1/2r_s)^3, r_s in the kernels' length unit (Ctx::pscale), and round once; Horner order (highest
+    // degree first)
+    const long double rs = (long double)c->r_s / (long double)c->pscale;
+    const long double k3 = 1.0L / (8.0L * rs * rs * rs);
     c->poly_deg = deg;
     for (int i = 0; i <= deg; ++i) c->poly_c[i] = (float)(mono[deg - i] * k3);
     return PHOTONS_OK;

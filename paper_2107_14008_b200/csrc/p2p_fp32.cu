@@ -22,25 +22,35 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     a.maxleaf = c->p.maxleaf; a.log2m = 0;
     while ((1 << a.log2m) < a.maxleaf) ++a.log2m;
     a.chunk_max = c->p.chunk_max; a.mixed = c->p.precision == PHOTONS_MIXED;
-    a.L = (float)c->p.boxsize; a.invL = (float)(1.0 / c->p.boxsize);
-    a.rcut2 = (float)(c->r_cut * c->r_cut);
-    a.rclose2 = (float)(c->p.close_pair_radius * c->p.close_pair_radius);
+    // kernel units: lengths / pscale, G m / gmscale (common.cuh); everything the pair core touches is O(1)
+    const double ps = c->pscale, ips = 1.0 / c->pscale;
+    const double Ls = c->p.boxsize * ips, rs = c->r_s * ips, rcut = c->r_cut * ips;
+    a.inv_pscale = ips;
+    a.oscale = c->gmscale * ips * ips;
+    a.inv_oscale = 1.0 / a.oscale;
+    a.Lh = (float)Ls; a.Ll = (float)(Ls - (double)a.Lh); a.invL = (float)(1.0 / Ls);
+    a.rcut2 = (float)(rcut * rcut);
+    const double eps = c->p.softening * ips;
+    a.r2add = std::fmax(R2_FLOOR, (float)(eps * eps));
+    a.eps2_d = c->p.softening * c->p.softening;
+    a.rclose2 = (float)(c->p.close_pair_radius * ips * c->p.close_pair_radius * ips);
+    if (!(a.rclose2 > 2.0f * a.r2add)) a.rclose2 = 0.f;      // nothing left to redo exactly inside the softening core
     a.Ld = c->p.boxsize; a.inv2rs_d = 1.0 / (2.0 * c->r_s);
-    // the fast path clamps at the fp32 value of r_close^2; the exact path uses the same radius
-    a.rclose_d = std::sqrt((double)a.rclose2);
+    // the fast path clamps at the fp32 value of r_close^2; the exact path uses the same radius (caller units)
+    a.rclose_d = std::sqrt((double)a.rclose2) * ps;
     a.wclose_d = 0.0;
     if (a.rclose_d > 0) {
         const double x = a.rclose_d * a.inv2rs_d;
         const double g = std::erfc(x) + 1.1283791670955125739 * x * std::exp(-x * x);
         a.wclose_d = g / (a.rclose_d * a.rclose_d * a.rclose_d);
     }
-    a.inv2rs = (float)a.inv2rs_d;
+    a.inv2rs = (float)(1.0 / (2.0 * rs));
     const double smax = 0.25 * c->p.rcut_over_rs * c->p.rcut_over_rs;
-    a.tk = (float)(2.0 / (smax * 4.0 * c->r_s * c->r_s));
+    a.tk = (float)(2.0 / (smax * 4.0 * rs * rs));
     for (int i = 0; i <= POLY_MAX_DEG; ++i) a.pc[i] = c->poly_c[i];
     a.tn = c->table.n;
     a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
-    a.uk = a.tn ? (float)(a.tn / 3.0 * a.inv2rs_d) : 0.f;
+    a.uk = a.tn ? (float)(a.tn / 3.0 / (2.0 * rs)) : 0.f;
     a.umax = (float)a.tn;
     a.table = c->table.d_TE;
     a.out = out; a.out_f32 = out_f32 ? 1 : 0;

@@ -10,6 +10,9 @@
 //                  one MUFU.RSQ per pair; sources are read as two broadcast LDS.128 per step
 //   accumulation   fp32 per staged run, flushed into fp64 per-lane sums (two-level, A12)
 //   close pairs    optional: pairs inside close_pair_radius are clamped in the fast path and redone in fp64
+//   units          lengths in units of Ctx::pscale (a power of two near r_cut), G m in units of Ctx::gmscale (a power
+//                  of two >= max |G m|): exact rescalings that keep every fp32 intermediate in range whatever the
+//                  caller's units are; the fp64 sums are scaled back when they are stored
 #pragma once
 #include "common.cuh"
 #include "pipeline.cuh"
@@ -25,7 +28,10 @@
 namespace photons {
 
 constexpr int MAX_RUN_LEAVES = 16;        // chunk_max / maxleaf at most (256 / 16)
-constexpr float R2_FLOOR = 1e-24f;       // added to every r^2: self / coincident pairs give w * 0 = 0 (A7)
+// Added to every r^2 (kernel length units, r_cut in [1, 2)): self / coincident pairs then give w * 0 = 0 with a finite
+// w (A7): 1/r^3 = 1e36 and G m <= 1 in kernel units, so w cannot overflow.  With Plummer softening (A23) eps^2 takes
+// its place.
+constexpr float R2_FLOOR = 1e-24f;
 constexpr float MAGIC = 12582912.0f;     // 1.5 * 2^23: float -> nearest-integer trick for the table index
 
 struct P32Args {
@@ -38,9 +44,13 @@ struct P32Args {
     const int* order;
     long long first;
     int maxleaf, log2m, chunk_max, mixed;
-    float L, invL, rcut2, rclose2;
-    double Ld, inv2rs_d, rclose_d, wclose_d;   // close pairs: g(r_close)/r_close^3 in fp64
-    float inv2rs;              // 1 / 2 r_s
+    float Lh, Ll, invL;        // box length in kernel units as an unevaluated sum of two floats (exact image shifts)
+    float rcut2, rclose2;      // kernel units; both compared with r^2 + r2add
+    float r2add;               // max(R2_FLOOR, eps^2): start value of every r^2 chain
+    double Ld, inv2rs_d, rclose_d, wclose_d, eps2_d;   // caller units (close pairs): g(r_close)/r_close^3 in fp64
+    double inv_pscale;         // 1 / Ctx::pscale
+    double oscale, inv_oscale; // kernel-unit sums -> caller units: gmscale / pscale^2
+    float inv2rs;              // 1 / 2 r_s (kernel units)
     float tk;                  // POLY: t = r2 * tk - 1
     float pc[POLY_MAX_DEG + 1];
     float uk, h, umax;         // TABLE: u = r * uk in node units, h = 3/n, umax = last node
@@ -51,7 +61,7 @@ struct P32Args {
 };
 
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
-// one MUFU.RSQ, no denormal fix-up code: r^2 carries R2_FLOOR, so it is never subnormal
+// one MUFU.RSQ, no denormal fix-up code: r^2 carries r2add >= R2_FLOOR, so it is never subnormal
 __device__ __forceinline__ float rsq(float x)
 {
     float y;
@@ -145,7 +155,7 @@ __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, f
 // kc: the loop constants (polynomial coefficients, tk, r_cut^2) as one local object
 struct LoopConst {
     float pc[POLY_MAX_DEG + 1];
-    float tk, rcut2;
+    float tk, rcut2, r2add;
 };
 
 template <int GKIND, int GPAR, int NCH>
@@ -178,10 +188,10 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
     }
 }
 
-// smallest r^2 seen so far, self / coincident pairs (r^2 == R2_FLOOR exactly) excluded: as unsigned integers
-// the bit patterns of positive floats keep their order, and subtracting bits(R2_FLOOR) + 1 wraps the
+// smallest r^2 seen so far, self / coincident pairs (r^2 == r2add exactly) excluded: as unsigned integers
+// the bit patterns of positive floats keep their order, and subtracting base = bits(r2add) + 1 wraps the
 // excluded value to the top (two ALU-pipe integer ops per pair instead of a compare, a select and a min)
-__device__ __forceinline__ unsigned close_key(float r2) { return (unsigned)__float_as_int(r2) - ((unsigned)__float_as_int(R2_FLOOR) + 1u); }
+__device__ __forceinline__ unsigned close_key(float r2, unsigned base) { return (unsigned)__float_as_int(r2) - base; }
 
 // exact weight difference for a close pair, fp64: G m_j [g(r)/r^3 - g(r_c)/r_c^3]
 static __device__ __noinline__ double close_pair_weight(double r2, double gm, double inv2rs, double wclose)
@@ -232,6 +242,8 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     }
     kc.tk = a.tk;
     kc.rcut2 = a.rcut2;
+    kc.r2add = a.r2add;
+    const unsigned ckbase = (unsigned)__float_as_int(a.r2add) + 1u;
 
     // targets -> registers (Alg. 1 L99)
     float tx[T], ty[T], tz[T];
@@ -280,10 +292,11 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             if (lane < nleaf) {
                 const long long jl = (long long)(e.x >> a.log2m) + lane;
                 const int sxi = (int)((e.y >> 16) & 3u) - 1, syi = (int)((e.y >> 18) & 3u) - 1, szi = (int)((e.y >> 20) & 3u) - 1;
-                cshift[st * MAX_RUN_LEAVES + lane] = make_float4((float)((a.ctr[3 * jl] + a.Ld * sxi) - cix),
-                                                                 (float)((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy),
-                                                                 (float)((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz), 0.f);
+                cshift[st * MAX_RUN_LEAVES + lane] = make_float4((float)(((a.ctr[3 * jl] + a.Ld * sxi) - cix) * a.inv_pscale),
+                                                                 (float)(((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy) * a.inv_pscale),
+                                                                 (float)(((a.ctr[3 * jl + 2] + a.Ld * szi) - ciz) * a.inv_pscale), 0.f);
             }
+            __syncwarp();   // the stores above are read by other lanes (first N_STAGES entries: before any loop barrier)
         }
         if (lane == 0) {
             const uint32_t bytes = (e.y & 0xffffu) * 16u;
@@ -321,14 +334,15 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 #pragma unroll
                 for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dc.x; qy[t] = ty[t] - dc.y; qz[t] = tz[t] - dc.z; }
             } else {
-                // s = +1: move the target by -L (exact, it sits in the upper half of the box);
-                // s = -1: move the sources by -L per pair (exact for the same reason)
-                sax = sxi < 0 ? -a.L : 0.f; say = syi < 0 ? -a.L : 0.f; saz = szi < 0 ? -a.L : 0.f;
+                // L = Lh + Ll (two floats).  s = +1: move the target by -L: t - Lh is exact (it sits in the upper half
+                // of the box), then - Ll; s = -1: move the sources by -Lh per pair (exact for the same reason) and
+                // the target by +Ll.  With a box length that fp32 holds exactly Ll = 0.
+                sax = sxi < 0 ? -a.Lh : 0.f; say = syi < 0 ? -a.Lh : 0.f; saz = szi < 0 ? -a.Lh : 0.f;
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    qx[t] = sxi > 0 ? tx[t] - a.L : tx[t];
-                    qy[t] = syi > 0 ? ty[t] - a.L : ty[t];
-                    qz[t] = szi > 0 ? tz[t] - a.L : tz[t];
+                    qx[t] = sxi > 0 ? (tx[t] - a.Lh) - a.Ll : sxi < 0 ? tx[t] + a.Ll : tx[t];
+                    qy[t] = syi > 0 ? (ty[t] - a.Lh) - a.Ll : syi < 0 ? ty[t] + a.Ll : ty[t];
+                    qz[t] = szi > 0 ? (tz[t] - a.Lh) - a.Ll : szi < 0 ? tz[t] + a.Ll : tz[t];
                 }
             }
             const bool seam = (sax != 0.f) | (say != 0.f) | (saz != 0.f);
@@ -344,9 +358,12 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 #pragma unroll
                         for (int hh = 0; hh < 2; ++hh) {
                             float dx = (hh ? A.y : A.x) - qx[t], dy = (hh ? A.w : A.z) - qy[t], dz = (hh ? B.y : B.x) - qz[t];
-                            dx -= a.L * rintf(dx * a.invL); dy -= a.L * rintf(dy * a.invL); dz -= a.L * rintf(dz * a.invL);
-                            float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, R2_FLOOR)));
-                            if (CLOSE) { kmin = min(kmin, close_key(r2)); r2 = fmaxf(r2, a.rclose2); }
+                            const float ix = rintf(dx * a.invL), iy = rintf(dy * a.invL), iz = rintf(dz * a.invL);
+                            dx = fmaf(-a.Ll, ix, fmaf(-a.Lh, ix, dx));
+                            dy = fmaf(-a.Ll, iy, fmaf(-a.Lh, iy, dy));
+                            dz = fmaf(-a.Ll, iz, fmaf(-a.Lh, iz, dz));
+                            float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.r2add)));
+                            if (CLOSE) { kmin = min(kmin, close_key(r2, ckbase)); r2 = fmaxf(r2, a.rclose2); }
                             const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
                         }
@@ -380,9 +397,9 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                     }
 #pragma unroll
                     for (int c = 0; c < NCH; ++c) {
-                        r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(R2_FLOOR))));
+                        r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(kc.r2add))));
                         if (CLOSE) {
-                            kmin = min(kmin, min(close_key(r2[c].x), close_key(r2[c].y)));
+                            kmin = min(kmin, min(close_key(r2[c].x, ckbase), close_key(r2[c].y, ckbase)));
                             r2[c] = f2(fmaxf(r2[c].x, a.rclose2), fmaxf(r2[c].y, a.rclose2));
                         }
                     }
@@ -418,7 +435,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
             // The fast path evaluated pairs inside r_close as if they sat at r_close.  Redo those pairs in
             // fp64 from the exact coordinates.  Self pairs do not trigger the scan (close_key), so it runs
             // only for runs that really hold a close pair.
-            if (__any_sync(0xffffffffu, kmin < close_key(a.rclose2))) {
+            if (__any_sync(0xffffffffu, kmin < close_key(a.rclose2, ckbase))) {
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     const double4 pi = a.p64[tslot[t]];
@@ -431,8 +448,9 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                             dx += a.Ld * sxi; dy += a.Ld * syi; dz += a.Ld * szi;
                         }
                         const double r2 = dx * dx + dy * dy + dz * dz;
-                        if (r2 > 0.0 && r2 < a.rclose_d * a.rclose_d) {
-                            const double w = close_pair_weight(r2, pj.w, a.inv2rs_d, a.wclose_d);
+                        const double r2e = r2 + a.eps2_d;
+                        if (r2 > 0.0 && r2e < a.rclose_d * a.rclose_d) {
+                            const double w = close_pair_weight(r2e, pj.w, a.inv2rs_d, a.wclose_d) * a.inv_oscale;
                             ax[t] += w * dx; ay[t] += w * dy; az[t] += w * dz;
                         }
                     }
@@ -474,12 +492,14 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         if (lane >= LG) continue;
         const int dst = a.slot_src[tslot[t]];
         if (dst < 0) continue;
+        // back to the caller's units (a power of two: exact)
+        const double ox = ax[t] * a.oscale, oy = ay[t] * a.oscale, oz = az[t] * a.oscale;
         if (a.out_f32) {
             float* o = reinterpret_cast<float*>(a.out) + 3 * (size_t)dst;
-            o[0] = (float)ax[t]; o[1] = (float)ay[t]; o[2] = (float)az[t];
+            o[0] = (float)ox; o[1] = (float)oy; o[2] = (float)oz;
         } else {
             double* o = reinterpret_cast<double*>(a.out) + 3 * (size_t)dst;
-            o[0] = ax[t]; o[1] = ay[t]; o[2] = az[t];
+            o[0] = ox; o[1] = oy; o[2] = oz;
         }
     }
 }
@@ -508,7 +528,7 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
         default: return fail(c, PHOTONS_EINVAL, "targets_per_lane %d is not available for maxleaf %d", T, M);
     }
 #undef PH_SHAPE
-    PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PH_CUDA(c, opt_in_smem(c, reinterpret_cast<const void*>(kern), smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
     ++c->launches;
     PH_CUDA(c, cudaGetLastError());
@@ -518,8 +538,8 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
 template <int GKIND, int GPAR>
 static int launch_p32_close(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
 {
-    return a.rclose2 > 1e-20f ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
-                                      : launch_p32_shape<GKIND, GPAR, false>(c, a, count, st);
+    return a.rclose2 > 0.f ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
+                           : launch_p32_shape<GKIND, GPAR, false>(c, a, count, st);
 }
 
 int launch_p32_poly(Ctx* c, const P32Args& a, long long count, cudaStream_t st);

@@ -1,10 +1,31 @@
 // fp64 P2P kernel (Alg. 1 + Alg. 2, the paper's DP run L196): one CTA per target leaf, the CTA's
 // warps split the leaf's source list, lanes own targets, source runs arrive in shared memory by TMA bulk
 // copies through a per-warp mbarrier ring (pipeline.cuh).  SURVEY.md §8(a) steps a4-a9.
+//
+// The pair core is bound by the FP64 pipe (64 lanes per SM: a warp-wide DFMA/DADD/DMUL/DSETP holds a scheduler's
+// DP unit for two cycles), so the design rule is: as few DP-pipe instructions per pair as the tolerance allows.
+//   - branch-free: self / coincident pairs are neutralised by a tiny start value of the r^2 chain (w * 0 = 0 with a
+//     finite w), the cut is one DSETP + a select on the weight;
+//   - 1/r from MUFU.RSQ64H (XU pipe, ~20 bits) and ONE third-order correction step (5 DP ops, error ~ e^3 = 2^-60)
+//     instead of the library's rsqrt (two Newton steps plus special-case code, ~12 DP ops);
+//   - U independent source chains per lane so that the dependent DFMA chains of one pair overlap with the others';
+//   - the interpolation table lives in shared memory, in one of two layouts:
+//       paper layout  {T_i, E_i}, Eq. 2's polynomials in x_i rebuilt per pair (L129-L151: 14 flops in the paper's count);
+//       coefficient layout  c_k = T^(k)(x_i) h^k / k!, k = 0..level, per node: the same Taylor series about the same
+//         node with the node polynomials folded in when the table is built (Horner only: `level` DFMAs).  The paper
+//         tabulates two numbers per node "considering the suitable capacity of shared memory" (L143, 96 KB on V100);
+//         with 227 KB per SM on B200 the 5-column table of 512 nodes (20 KB) is the cheaper trade.
+//   - index by the magic-number add in fp64 (the low word of u + 1.5 * 2^52 is the nearest integer): no F2I/I2F.
 #include "common.cuh"
 #include "pipeline.cuh"
 
 namespace photons {
+
+constexpr double R2_FLOOR64 = 0x1p-600;   // start of every r^2 chain: 1/r^3 = 2^900 stays finite, w * 0 = 0 (A7)
+constexpr double MAGIC64 = 6755399441055744.0;   // 1.5 * 2^52
+constexpr int TAB_STRIDE = 5;             // doubles per node in the coefficient layout (odd: fewer bank conflicts)
+
+enum { G64_DIRECT = 0, G64_TABLE = 1, G64_COEF = 2 };
 
 struct P64Args {
     const double4* p64;       // n_slots x {x, y, z, G m}
@@ -14,9 +35,10 @@ struct P64Args {
     const int* order;         // CTA b works on leaf order[first + b]
     long long first;
     int maxleaf, chunk_max;
-    double L, rcut2, inv2rs;
-    const double2* table;     // TABLE mode: {T_i, E_i}, i = 0..tn
-    int tn;
+    double L, rcut2, inv2rs, r2add;
+    const double* table;      // TABLE: {T_i, E_i} pairs; COEF: TAB_STRIDE doubles per node; i = 0..tn
+    int tn, tab_doubles;      // number of doubles to stage in shared memory
+    double uk, h;             // u = r * uk in node units; h = 3 / tn
     void* out;                // caller order, n x 3
     int out_f32;
 };
@@ -27,27 +49,64 @@ __device__ __forceinline__ double g_direct64(double x)
     return erfc(x) + 1.1283791670955125739 * x * exp(-x * x);
 }
 
-// Eq. 2 to level LEVEL about the nearest node (A14)
-template <int LEVEL>
-__device__ __forceinline__ double g_table64(double x, const double2* __restrict__ table, int tn)
+// 1/sqrt(x) for normal positive x: MUFU.RSQ64H seed on the high word, then y (1 + e/2 + 3 e^2/8), e = 1 - x y^2
+__device__ __forceinline__ double rsqrt64(double x)
 {
-    const double h = 3.0 / tn;
-    int i = (int)rint(x * (tn / 3.0));
-    i = min(i, tn);
-    const double xi = i * h;
-    const double e = x - xi;
-    const double2 te = __ldg(&table[i]);
-    const double Ti = te.x, Ei = te.y;
-    const double xi2 = xi * xi;
-    double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1), Horner from the highest kept level
-    if (LEVEL >= 4) poly = -xi * (xi2 * xi2 * (1.0 / 3.0) - 1.5 * xi2 + 1.0);
-    if (LEVEL >= 3) poly = poly * e + ((2.0 / 3.0) * xi2 * xi2 - (5.0 / 3.0) * xi2 + (1.0 / 3.0));
-    if (LEVEL >= 2) poly = poly * e - xi * (xi2 - 1.0);
-    if (LEVEL >= 1) poly = poly * e + xi2;
-    return LEVEL >= 1 ? Ti + Ei * e * poly : Ti;
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double hx = x * y;
+    const double e = fma(-hx, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(y, e * p, y);
 }
 
-template <int T, int GMODE, int LEVEL>
+// g(x) for NCH chains at once; r = r2 * idr is passed in
+template <int GMODE, int LEVEL, int NCH>
+__device__ __forceinline__ void g_eval(const P64Args& a, const double* __restrict__ tab, const double (&r)[NCH], double (&g)[NCH])
+{
+    if constexpr (GMODE == G64_DIRECT) {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) g[c] = g_direct64(r[c] * a.inv2rs);
+    } else {
+    double eu[NCH], fi[NCH];
+    int idx[NCH];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+        const double u = r[c] * a.uk;                  // node units
+        const double um = u + MAGIC64;                 // nearest node (A14)
+        fi[c] = um - MAGIC64;
+        eu[c] = u - fi[c];                             // |eu| <= 1/2
+        idx[c] = min(__double2loint(um), a.tn);        // beyond the table only for pairs the cut discards anyway
+    }
+    if (GMODE == G64_COEF) {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const double* t = tab + idx[c] * TAB_STRIDE;
+            double p = t[LEVEL];
+#pragma unroll
+            for (int k = LEVEL - 1; k >= 0; --k) p = fma(p, eu[c], t[k]);
+            g[c] = p;
+        }
+    } else {
+        // Eq. 2 to level LEVEL about the nearest node, the node polynomials rebuilt from x_i
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const double2 te = reinterpret_cast<const double2*>(tab)[idx[c]];
+            const double xi = fi[c] * a.h, e = eu[c] * a.h;
+            const double xi2 = xi * xi;
+            double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1), Horner from the highest kept level
+            if (LEVEL >= 4) poly = -xi * fma(fma(xi2, 1.0 / 3.0, -1.5), xi2, 1.0);
+            if (LEVEL >= 3) poly = fma(poly, e, fma(fma(xi2, 2.0 / 3.0, -5.0 / 3.0), xi2, 1.0 / 3.0));
+            if (LEVEL >= 2) poly = fma(poly, e, fma(-xi, xi2, xi));
+            if (LEVEL >= 1) poly = fma(poly, e, xi2);
+            g[c] = LEVEL >= 1 ? fma(te.y * e, poly, te.x) : te.x;
+        }
+    }
+    }
+}
+
+// LG lanes own the leaf's targets (T per lane); with LG = 16 the two half-warps take alternate sources
+template <int T, int LG, int GMODE, int LEVEL>
 __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -59,17 +118,25 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
     uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES;
     uint2* meta = reinterpret_cast<uint2*>(tail + W * N_STAGES * 8) + warp * N_STAGES;
     double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 16);   // W x T x 32 x 3 doubles
+    double* tab = red + (size_t)W * T * 32 * 3;
+
+    constexpr int HS = 32 / LG;
+    const int half = HS > 1 ? lane / LG : 0;
+
+    if (GMODE != G64_DIRECT) {   // the interpolation table lives in shared memory (Fig. 1)
+        for (int i = threadIdx.x; i < a.tab_doubles; i += blockDim.x) tab[i] = a.table[i];
+        __syncthreads();
+    }
 
     const long long leaf = a.order[a.first + blockIdx.x];
     const long long slot0 = leaf * M;
 
     double tx[T], ty[T], tz[T], ax[T], ay[T], az[T];
-    bool live[T];
+    int tslot[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        const int l = lane + 32 * t;
-        live[t] = l < M;
-        const double4 p = a.p64[slot0 + (live[t] ? l : 0)];
+        tslot[t] = (int)slot0 + (lane % LG) + LG * t;
+        const double4 p = a.p64[tslot[t]];
         tx[t] = p.x; ty[t] = p.y; tz[t] = p.z;
         ax[t] = ay[t] = az[t] = 0.0;
     }
@@ -114,26 +181,45 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
             px[t] = py[t] = pz[t] = 0.0;
             qx[t] = tx[t] - sx; qy[t] = ty[t] - sy; qz[t] = tz[t] - sz;
         }
-        for (int j = 0; j < ns; ++j) {
-            const double4 s = src[j];
+        // U sources x T targets = NCH independent chains per iteration (ns is a multiple of maxleaf >= 16)
+        constexpr int U = T == 1 ? 4 : T == 2 ? 2 : 1;
+        constexpr int NCH = U * T;
+        auto step = [&](const int j, const bool image) {
+            double dx[NCH], dy[NCH], dz[NCH], r2[NCH], r[NCH], idr[NCH], gm[NCH], g[NCH];
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                double dx = s.x - qx[t], dy = s.y - qy[t], dz = s.z - qz[t];
-                if (per_pair) {
-                    dx -= a.L * rint(dx / a.L);
-                    dy -= a.L * rint(dy / a.L);
-                    dz -= a.L * rint(dz / a.L);
-                }
-                const double r2 = dx * dx + dy * dy + dz * dz;
-                if (r2 < a.rcut2 && r2 > 0.0) {
-                    const double idr = rsqrt(r2);
-                    const double r = r2 * idr;
-                    const double x = r * a.inv2rs;
-                    const double g = GMODE == PHOTONS_G_DIRECT ? g_direct64(x) : g_table64<LEVEL>(x, a.table, a.tn);
-                    const double w = s.w * g * (idr * idr * idr);
-                    px[t] += w * dx; py[t] += w * dy; pz[t] += w * dz;
+            for (int u = 0; u < U; ++u) {
+                const double4 s = src[j + u * HS];
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    const int c = u * T + t;
+                    dx[c] = s.x - qx[t]; dy[c] = s.y - qy[t]; dz[c] = s.z - qz[t];
+                    if (image) {      // degenerate geometry (tiny N): minimum image per pair
+                        dx[c] -= a.L * rint(dx[c] / a.L);
+                        dy[c] -= a.L * rint(dy[c] / a.L);
+                        dz[c] -= a.L * rint(dz[c] / a.L);
+                    }
+                    gm[c] = s.w;
                 }
             }
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                r2[c] = fma(dx[c], dx[c], fma(dy[c], dy[c], fma(dz[c], dz[c], a.r2add)));
+                idr[c] = rsqrt64(r2[c]);
+                r[c] = r2[c] * idr[c];
+            }
+            g_eval<GMODE, LEVEL, NCH>(a, tab, r, g);
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                const double v = (gm[c] * idr[c]) * (idr[c] * idr[c]) * g[c];
+                const double w = r2[c] < a.rcut2 ? v : 0.0;      // the cut (A8); also drops what g did beyond its range
+                const int t = c % T;
+                px[t] = fma(w, dx[c], px[t]); py[t] = fma(w, dy[c], py[t]); pz[t] = fma(w, dz[c], pz[t]);
+            }
+        };
+        if (per_pair) {
+            for (int j = half; j < ns; j += HS * U) step(j, true);
+        } else {
+            for (int j = half; j < ns; j += HS * U) step(j, false);
         }
 #pragma unroll
         for (int t = 0; t < T; ++t) { ax[t] += px[t]; ay[t] += py[t]; az[t] += pz[t]; }
@@ -141,27 +227,36 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
         if (lane == 0 && k + N_STAGES < n_my) issue(k + N_STAGES);
     }
 
+#pragma unroll
+    for (int o = 16; o >= LG; o >>= 1) {     // add the half-warps' partial sums (fixed order)
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            ax[t] += __shfl_xor_sync(0xffffffffu, ax[t], o);
+            ay[t] += __shfl_xor_sync(0xffffffffu, ay[t], o);
+            az[t] += __shfl_xor_sync(0xffffffffu, az[t], o);
+        }
+    }
     // sum the warps' partial accelerations (fixed order: deterministic), then scatter to caller order
     if (W > 1) {
 #pragma unroll
         for (int t = 0; t < T; ++t) {
-            double* r = red + ((size_t)(warp * T + t) * 32 + lane) * 3;
-            r[0] = ax[t]; r[1] = ay[t]; r[2] = az[t];
+            double* rr = red + ((size_t)(warp * T + t) * 32 + lane) * 3;
+            rr[0] = ax[t]; rr[1] = ay[t]; rr[2] = az[t];
         }
         __syncthreads();
         if (warp != 0) return;
 #pragma unroll
         for (int t = 0; t < T; ++t) {
             for (int w = 1; w < W; ++w) {
-                const double* r = red + ((size_t)(w * T + t) * 32 + lane) * 3;
-                ax[t] += r[0]; ay[t] += r[1]; az[t] += r[2];
+                const double* rr = red + ((size_t)(w * T + t) * 32 + lane) * 3;
+                ax[t] += rr[0]; ay[t] += rr[1]; az[t] += rr[2];
             }
         }
     }
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        if (!live[t]) continue;
-        const int dst = a.slot_src[slot0 + lane + 32 * t];
+        if (lane >= LG) continue;
+        const int dst = a.slot_src[tslot[t]];
         if (dst < 0) continue;
         if (a.out_f32) {
             float* o = reinterpret_cast<float*>(a.out) + 3 * (size_t)dst;
@@ -173,28 +268,36 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
     }
 }
 
-template <int T, int GMODE, int LEVEL>
+template <int T, int LG, int GMODE, int LEVEL>
 static int launch_t(Ctx* c, const P64Args& a, long long count, int W, size_t smem, cudaStream_t st)
 {
-    auto kern = p2p_fp64_kernel<T, GMODE, LEVEL>;
-    PH_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    auto kern = p2p_fp64_kernel<T, LG, GMODE, LEVEL>;
+    if (smem > 227 * 1024) return fail(c, PHOTONS_EINVAL, "fp64 kernel: %zu bytes of shared memory (ring + table) exceed 227 KB; use a smaller table or chunk_max", smem);
+    PH_CUDA(c, opt_in_smem(c, reinterpret_cast<const void*>(kern), smem));
     kern<<<(unsigned)count, 32 * W, smem, st>>>(a);
     ++c->launches;
     PH_CUDA(c, cudaGetLastError());
     return PHOTONS_OK;
 }
 
-template <int T>
+template <int T, int LG, int GMODE>
+static int launch_l(Ctx* c, const P64Args& a, long long count, int W, size_t smem, cudaStream_t st)
+{
+    switch (c->p.table_level) {
+        case 0: return launch_t<T, LG, GMODE, 0>(c, a, count, W, smem, st);
+        case 1: return launch_t<T, LG, GMODE, 1>(c, a, count, W, smem, st);
+        case 2: return launch_t<T, LG, GMODE, 2>(c, a, count, W, smem, st);
+        case 3: return launch_t<T, LG, GMODE, 3>(c, a, count, W, smem, st);
+        default: return launch_t<T, LG, GMODE, 4>(c, a, count, W, smem, st);
+    }
+}
+
+template <int T, int LG>
 static int launch_g(Ctx* c, const P64Args& a, long long count, int W, size_t smem, cudaStream_t st)
 {
-    if (c->p.g_mode == PHOTONS_G_DIRECT) return launch_t<T, PHOTONS_G_DIRECT, 0>(c, a, count, W, smem, st);
-    switch (c->p.table_level) {
-        case 0: return launch_t<T, PHOTONS_G_TABLE, 0>(c, a, count, W, smem, st);
-        case 1: return launch_t<T, PHOTONS_G_TABLE, 1>(c, a, count, W, smem, st);
-        case 2: return launch_t<T, PHOTONS_G_TABLE, 2>(c, a, count, W, smem, st);
-        case 3: return launch_t<T, PHOTONS_G_TABLE, 3>(c, a, count, W, smem, st);
-        default: return launch_t<T, PHOTONS_G_TABLE, 4>(c, a, count, W, smem, st);
-    }
+    if (c->p.g_mode == PHOTONS_G_DIRECT) return launch_t<T, LG, G64_DIRECT, 0>(c, a, count, W, smem, st);
+    if (c->p.table_layout == PHOTONS_TABLE_COEF) return launch_l<T, LG, G64_COEF>(c, a, count, W, smem, st);
+    return launch_l<T, LG, G64_TABLE>(c, a, count, W, smem, st);
 }
 
 int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st)
@@ -203,14 +306,29 @@ int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool ou
     a.p64 = c->d_p64; a.slot_src = c->d_slot_src; a.chunk_ptr = c->d_chunk_ptr; a.chunks = c->d_chunks;
     a.order = c->d_order; a.first = first; a.maxleaf = c->p.maxleaf; a.chunk_max = c->p.chunk_max;
     a.L = c->p.boxsize; a.rcut2 = c->r_cut * c->r_cut; a.inv2rs = 1.0 / (2.0 * c->r_s);
-    a.table = c->table.d_TE64; a.tn = c->table.n; a.out = out; a.out_f32 = out_f32 ? 1 : 0;
+    // start value of the r^2 chain: eps^2 (A23), else a floor far below any separation, scaled with r_cut^2 so that
+    // it means the same in any units
+    a.r2add = c->p.softening > 0 ? c->p.softening * c->p.softening : R2_FLOOR64 * a.rcut2;
+    const bool coef = c->p.table_layout == PHOTONS_TABLE_COEF;
+    a.table = nullptr; a.tn = 0; a.tab_doubles = 0;
+    if (c->p.g_mode == PHOTONS_G_TABLE) {
+        a.tn = c->table.n;
+        a.table = coef ? c->table.d_C64 : reinterpret_cast<const double*>(c->table.d_TE64);
+        a.tab_doubles = (a.tn + 1) * (coef ? TAB_STRIDE : 2);
+        a.h = 3.0 / a.tn;
+        a.uk = a.tn / 3.0 * a.inv2rs;
+    }
+    a.out = out; a.out_f32 = out_f32 ? 1 : 0;
     const int W = c->p.warps_per_leaf;
-    const int T = (c->p.maxleaf + 31) / 32;
-    const size_t smem = (size_t)W * N_STAGES * c->p.chunk_max * 32 + (size_t)W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8;
-    switch (T) {
-        case 1: return launch_g<1>(c, a, count, W, smem, st);
-        case 2: return launch_g<2>(c, a, count, W, smem, st);
-        default: return launch_g<4>(c, a, count, W, smem, st);
+    const int M = c->p.maxleaf;
+    const int T = (M + 31) / 32;
+    const size_t smem = (size_t)W * N_STAGES * c->p.chunk_max * 32 + (size_t)W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8 +
+                        (size_t)a.tab_doubles * 8;
+    switch (M) {
+        case 16: return launch_g<1, 16>(c, a, count, W, smem, st);
+        case 32: return launch_g<1, 32>(c, a, count, W, smem, st);
+        case 64: return launch_g<2, 32>(c, a, count, W, smem, st);
+        default: return launch_g<4, 32>(c, a, count, W, smem, st);
     }
 }
 

@@ -37,41 +37,27 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, float a_in, floa
         } else if (KIND == 3) {     // MUFU.RSQ
 #pragma unroll
             for (int i = 0; i < CH; ++i) x[i] = rsqrtf(x[i]);
-        } else if (KIND == 4) {     // 8 FFMA2 : 2 MUFU.RSQ (the pair core's ratio is about 15 : 2)
-#pragma unroll
-            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], a2, b2);
-            x[0] = rsqrtf(x[0]);
-            x[1] = rsqrtf(x[1]);
         } else if (KIND == 5) {     // LDS.128, one address per warp (broadcast)
 #pragma unroll
             for (int i = 0; i < CH; ++i) {
                 const float4 v = sh[(it + i) & 63];
                 acc4.x += v.x; acc4.y += v.y; acc4.z += v.z; acc4.w += v.w;
             }
-        } else if (KIND == 6) {     // FFMA with immediate operands
-#pragma unroll
-            for (int i = 0; i < CH; ++i) x[i] = fmaf(x[i], 0.999f, 0.001f);
-        } else if (KIND == 7) {     // 8 FFMA2 : 4 ALU-pipe ops (compare-to-float, min)
-#pragma unroll
-            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], a2, b2);
-            x[0] = x[0] < a ? 1.f : 0.f;
-            x[1] = fminf(x[1], b);
-            x[2] = x[2] < b ? 1.f : 0.f;
-            x[3] = fmaxf(x[3], a);
         } else if (KIND == 8) {     // FADD2
 #pragma unroll
             for (int i = 0; i < CH / 2; ++i) y[i] = __fadd2_rn(y[i], a2);
         } else if (KIND == 9) {     // FMUL2
 #pragma unroll
             for (int i = 0; i < CH / 2; ++i) y[i] = __fmul2_rn(y[i], a2);
-        } else if (KIND == 10) {    // FFMA2 with both multiplicands distinct per chain (no operand reuse)
+        } else if (KIND == 4) {     // MUFU.EX2
 #pragma unroll
-            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
-        } else if (KIND == 16 || KIND == 17) {   // 8 FFMA2 without operand reuse : 4 (16) or 8 (17) ALU-pipe ops
+            for (int i = 0; i < CH; ++i) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(x[i]));
+        } else if (KIND == 6) {     // DADD
 #pragma unroll
-            for (int i = 0; i < CH / 2; ++i) y[i] = __ffma2_rn(y[i], y[(i + 1) % (CH / 2)], b2);
+            for (int i = 0; i < CH / 2; ++i) d[i] = d[i] + (double)a;
+        } else if (KIND == 7) {     // MUFU.RSQ64H (the seed of the fp64 kernel's reciprocal square root)
 #pragma unroll
-            for (int i = 0; i < (KIND == 16 ? 4 : 8); ++i) x[i] = __int_as_float(__float_as_int(x[i]) ^ (it + i));
+            for (int i = 0; i < CH / 2; ++i) asm volatile("rsqrt.approx.ftz.f64 %0, %0;" : "+d"(d[i]));
         } else if (KIND >= 11 && KIND <= 15) {
             // the pair core's instruction mix per step (two pairs per lane): 24 FFMA2-class in two dependent
             // chains (Horner), plus 11: 2 MUFU.RSQ (single instruction, ftz)   12: + 2 x (FSETP + FSEL)
@@ -137,7 +123,8 @@ extern "C" int photons_peak_probe(int device, int kind, double* out)
     // kind + 100 * b: the same probe with only b (1..7) resident blocks of 8 warps per SM (occupancy sweep)
     g_blocks_per_sm = 8;
     if (kind >= 100) { g_blocks_per_sm = kind / 100; kind %= 100; }
-    if (!out || kind < 0 || kind > 17 || g_blocks_per_sm < 1 || g_blocks_per_sm > 8) return PHOTONS_EINVAL;
+    const bool known = (kind >= 0 && kind <= 9) || (kind >= 11 && kind <= 15);
+    if (!out || !known || g_blocks_per_sm < 1 || g_blocks_per_sm > 8) return PHOTONS_EINVAL;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) {
         cudaGetLastError();
@@ -153,20 +140,17 @@ extern "C" int photons_peak_probe(int device, int kind, double* out)
         case 1: e = run_probe<1>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
         case 2: e = run_probe<2>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH / 2; break;
         case 3: e = run_probe<3>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
-        case 4: e = run_probe<4>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // counts the FFMA2 lanes only
+        case 4: e = run_probe<4>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
         case 5: e = run_probe<5>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // LDS.128 per lane
-        case 6: e = run_probe<6>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
-        case 7: e = run_probe<7>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;     // counts the FFMA2 lanes only
+        case 6: e = run_probe<6>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH / 2; break;
+        case 7: e = run_probe<7>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH / 2; break;
         case 8: e = run_probe<8>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
         case 9: e = run_probe<9>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
-        case 10: e = run_probe<10>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
         case 11: e = run_probe<11>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
         case 12: e = run_probe<12>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
         case 13: e = run_probe<13>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
         case 14: e = run_probe<14>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
-        case 15: e = run_probe<15>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
-        case 16: e = run_probe<16>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
-        default: e = run_probe<17>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = CH; break;
+        default: e = run_probe<15>(prop.multiProcessorCount, d_out, &ms); lane_ops_per_thread_iter = 48; break;
     }
     cudaFree(d_out);
     if (e != cudaSuccess) return PHOTONS_ECUDA;
