@@ -40,24 +40,55 @@ from paper_2107_14008_b200 import workloads  # noqa: E402
 METRIC = "truncated P2P pair interactions/s (evaluated pairs, fp32 path)"
 UNIT = "pairs/s"
 
-# B200 FP32 vector peak: SMs x FP32 lanes x 2 flop x max SM clock
+# B200 vector peaks: SMs x lanes x 2 flop x max SM clock
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128
-# executed flops per evaluated pair of the headline kernel, FFMA = 2, FADD/FMUL/MUFU = 1, counted from its
-# SASS inner loop: poly g of degree d -> (8 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
+FP64_LANES_PER_SM = 64
 POLY_DEGREE = 12               # the library's default (photons_params.poly_degree = 0)
-
-
-def flops_per_pair(g_mode: str, poly_degree: int = POLY_DEGREE) -> float:
-    if g_mode == "poly":
-        return 2.0 * (8 + poly_degree) + 3 + 2 + 1
-    if g_mode == "table":      # 512 nodes, level 2: 9 FFMA + 6 FADD + 10 FMUL + 1 MUFU
-        return 2.0 * 9 + 6 + 10 + 1
-    return 51.0                # direct: the paper's convention; erfcf/expf are not itemised
 PAPER_FLOPS_PER_PAIR = 51.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the headline kernel, from the committed
-# `ncu --set full` capture (profiles/r1_p2p_fp32_poly12_ncu_full.md): config 4, MAXLEAF 32, fp32, poly.
-NCU_TRAFFIC_BYTES = {("c4_clustered_256", 32, "fp32", "poly"): 20.127754e9 + 0.671901440e9}
+
+
+def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGREE, table_level: int = 2,
+                   table_layout: str = "paper") -> float:
+    """Executed flops per evaluated pair, counted in the SASS of each kernel's hot loop (profiles/r2_sass_inner_loop.md;
+    ncu's op_ffma counters read 0 for the packed FFMA2 stream): FFMA/DFMA = 2, FADD/FMUL/DADD/DMUL = 1, MUFU = 1,
+    compares and selects 0."""
+    if precision == "fp64":
+        if g_mode == "direct":     # 74 DFMA + 17 DMUL + 12 DADD + 3 MUFU (library erfc + exp inlined, branch-free)
+            return 2.0 * 74 + 17 + 12 + 3
+        if table_layout == "coef":  # level 4: 15 DFMA + 7 DMUL + 4 DADD + 1 MUFU; one DFMA per level
+            return 2.0 * (11 + table_level) + 7 + 4 + 1
+        # paper layout: level 4: 20 DFMA + 12 DMUL + 4 DADD + 1 MUFU; level 3: 18 + 11 + 4 + 1
+        return {4: 57.0, 3: 52.0}.get(table_level, 52.0 - 4.0 * (3 - table_level))
+    if g_mode == "poly":           # (8 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
+        return 2.0 * (8 + poly_degree) + 3 + 2 + 1
+    if g_mode == "table":          # 512 nodes, level 2: 9 FFMA + 6 FADD + 10 FMUL + 1 MUFU
+        return 2.0 * 9 + 6 + 10 + 1 + 2.0 * (table_level - 2)
+    if g_mode == "fused":          # hand-fused erfc/exp: see profiles/r2_sass_inner_loop.md
+        return FUSED_FLOPS_PER_PAIR
+    # direct = stock erfcf + expf: 31 FFMA + 16 FMUL + 8.5 FADD + 5 MUFU (3 FFMA2 + 1.5 FADD2 packed among them)
+    return 2.0 * 31 + 16 + 8.5 + 5
+
+
+FUSED_FLOPS_PER_PAIR = 2.0 * (7 + 10) + 8 + 3 + 2   # degree 10: 17 FFMA + 8 FMUL + 3 FADD + MUFU.RSQ + MUFU.EX2
+
+
+def peak_tflops(precision: str, sm_mhz: float) -> float:
+    lanes = FP64_LANES_PER_SM if precision == "fp64" else FP32_LANES_PER_SM
+    return SM_COUNT * lanes * 2 * sm_mhz * 1e6 / 1e12
+
+
+def ncu_traffic(workload: str, maxleaf: int, precision: str, g_mode: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed `ncu --set
+    full` summaries (profiles/r2_traffic.json, each entry naming its capture and commit); null when this variant has
+    none.  Never a number typed in here."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as f:
+            table = json.load(f)
+    except OSError:
+        return None, None
+    e = table.get(f"{workload}/{maxleaf}/{precision}/{g_mode}")
+    return (e["dram_bytes"], e["source"]) if e else (None, None)
 
 
 def geometry(cfg):
@@ -65,11 +96,13 @@ def geometry(cfg):
     return r_s, 6.0 * r_s                   # r_cut = 6 r_s (north_star)
 
 
-# Radius (in r_cut) inside which fp32 pairs are redone in fp64 (A12), per workload kind: pairs closer
-# than about sqrt(G m / 1.5 a_rms) carry more than the whole rms acceleration.  Uniform-like loads need it to
-# meet 1e-5 * rms in the max norm (max|a|/rms ~ 100); on the clustered loads the rms itself is set by the dense
-# cores (max/rms ~ 9) and plain fp32 already passes with 5x margin (tests/test_gpu_parity.py, full size).
-CLOSE_OVER_RCUT = {"uniform": 0.02, "grid": 0.02, "clustered": 0.0}
+# close_pair_radius (in r_cut) of the fp32 kernels' exact path (A12), per workload kind: a staged run whose fp32
+# partial acceleration exceeds G m / r_close^2 is redone in fp64.  The literal criterion max|da| <= 1e-5 rms needs it on
+# every load: the fp32 pair core is good to ~6e-7 relative (three times the rsqrt's 2 ulp), so a target whose
+# acceleration exceeds ~15 rms misses 1e-5 rms without it (config 4 at 10^4 targets: 2.1e-5 at |a| = 36 rms).  The radii
+# put the trigger at a few rms: uniform-like loads (rms ~ 32 G m / spacing^2) 0.02 r_cut = 2.9 rms; clustered loads, whose
+# rms is set by the dense cores, 5e-4 r_cut = 3-8 rms.  A run is redone for well under 1 % of the targets.
+CLOSE_OVER_RCUT = {"uniform": 0.02, "grid": 0.02, "clustered": 5e-4}
 
 
 def headline_params(cfg, **over):
@@ -169,8 +202,12 @@ def oracle_sample(cfg, pos, mass, seconds_target: float, n_threads_hint: int):
     import oracle
     oracle.build()
     r_s, r_cut = geometry(cfg)
-    # ~1.3e8 pair tests per second per core (measured on the first run; only sets the sample size)
-    n_t = int(max(64, min(cfg.n, seconds_target * 1.3e8 * n_threads_hint / cfg.n)))
+    # ~1.3e8 pair tests per second per core (measured on the first run; only sets the sample size).  The oracle hands
+    # out targets in chunks of 16 (schedule(dynamic, 16)): a whole number of rounds of chunks over the threads, and at
+    # least four rounds, so that the measured rate does not depend on the sample size (load balance).
+    quantum = 16 * max(1, n_threads_hint)
+    n_t = int(seconds_target * 1.3e8 * n_threads_hint / cfg.n)
+    n_t = min(cfg.n, max(4 * quantum, (n_t + quantum - 1) // quantum * quantum))
     tgt = workloads.sample_targets(cfg.n, n_t, cfg.seed)
     t0 = time.perf_counter()
     _, cnt = oracle.p2p_sampled(pos, mass, tgt, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut, G=cfg.G)
@@ -235,7 +272,15 @@ def run_ours(args):
     pos32 = pos.astype(np.float32)               # exact: the caller's data are fp32
     params = headline_params(cfg, device=local, n_streams=args.streams, g_mode=args.g_mode,
                              precision=args.precision, maxleaf=args.maxleaf or cfg.maxleaf)
-    if args.no_close:
+    if args.g_mode == "table":
+        params.update(table_nodes=args.table_nodes, table_level=args.table_level, table_layout=args.table_layout)
+    if args.softening_over_rcut:
+        params["softening"] = args.softening_over_rcut * r_cut
+    if args.warps_per_leaf:
+        params["warps_per_leaf"] = args.warps_per_leaf
+    if args.leaf_order:
+        params["leaf_order"] = args.leaf_order
+    if args.no_close or args.precision == "fp64":
         params["close_pair_radius"] = 0.0
     n = cfg.n
 
@@ -285,35 +330,41 @@ def run_ours(args):
     value = units / (ms_max * 1e-3)
 
     # end to end through the C ABI with host buffers
-    for _ in range(min(args.warmup, 2)):
-        step_host()
     e_steps = max(1, min(args.steps, 3))
-    e_ms, _, _, _, _ = timed(step_host, e_steps)
-    e_ms_max, e_units = aggregate(e_ms, pairs * e_steps, dist if world > 1 else None)
-    e2e_value = e_units / (e_ms_max * 1e-3)
+    if args.no_e2e:          # profiling runs only: the bench line then carries no end-to-end number
+        e_ms_max, e2e_value = float("nan"), None
+    else:
+        for _ in range(min(args.warmup, 2)):
+            step_host()
+        e_ms, _, _, _, _ = timed(step_host, e_steps)
+        e_ms_max, e_units = aggregate(e_ms, pairs * e_steps, dist if world > 1 else None)
+        e2e_value = e_units / (e_ms_max * 1e-3)
 
     line = None
     if rank == 0:
         kernel_ms = float(np.mean(k_ms))
-        fpp = flops_per_pair(args.g_mode)
+        fpp = flops_per_pair(args.precision, args.g_mode, table_level=args.table_level, table_layout=args.table_layout)
         clocks = clk.summary()
-        peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965.0) * 1e6 / 1e12
+        peak_tf = peak_tflops(args.precision, clocks["sm_max_mhz"] or 1965.0)
         achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
+        traffic, traffic_src = ncu_traffic(cfg0.name, params["maxleaf"], args.precision, args.g_mode)
+        f64 = args.precision == "fp64"
         roofline = {
-            "bound": "alu", "kernel": "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-            "frac": achieved_tf / peak_tf,
-            "traffic": NCU_TRAFFIC_BYTES.get((cfg0.name, params["maxleaf"], args.precision, args.g_mode)),
+            "bound": "alu", "kernel": "p2p_fp64_kernel" if f64 else "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf,
+            "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+            "traffic": traffic, "traffic_source": traffic_src,
             "traffic_unit": "bytes per launch (ncu dram read + write; the bound is ALU, not HBM)",
-            "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); "
-                           "MEASURED_PEAKS.json holds no FP32 vector peak",
+            "peak_source": f"derived: 148 SMs x {FP64_LANES_PER_SM if f64 else FP32_LANES_PER_SM} FP{'64' if f64 else '32'} lanes x 2 flop x "
+                           "clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no vector-ALU peak; photons_peak_probe measures "
+                           "0.89-0.91 (FFMA, FFMA2) and 0.87 (DFMA) of it (profiles/r2_peak_probe.md)",
             "flops_per_pair": fpp, "kernel_ms": kernel_ms, "kernel_pairs_per_s": pairs / (kernel_ms * 1e-3),
             "kernel_share_of_step": kernel_ms / (ms / args.steps),
-            "frac_at_sampled_clock": (achieved_tf / (SM_COUNT * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
-                                      if clocks["sm_mhz"] else None),
+            "frac_at_sampled_clock": (achieved_tf / peak_tflops(args.precision, clocks["sm_mhz"]) if clocks["sm_mhz"] else None),
             "paper_convention_tflops": pairs * PAPER_FLOPS_PER_PAIR / (kernel_ms * 1e-3) / 1e12,
         }
         # CPU baseline: the oracle on a bounded sample of the same workload, all host cores
         cpu = None
+        within_cut_total = None
         if not args.no_cpu_baseline:
             import oracle
             cores = oracle.num_threads()
@@ -322,6 +373,7 @@ def run_ours(args):
                    "sample": f"{n_t} seeded targets x all {n} sources, {secs:.1f} s (pair tests counted; "
                              f"within-cut pairs/s = {incut / secs:.3e})",
                    "within_cut_pairs_per_s": incut / secs}
+            within_cut_total = incut / n_t * n       # the sample's mean in-cut neighbour count x N
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -334,7 +386,11 @@ def run_ours(args):
                        "step": "set_particles + build_leaves + short_range_acc"},
             "pairs_evaluated_per_step": pairs, "n_leaf_pairs": st["n_leaf_pairs"], "n_chunks": st["n_chunks"],
             "build_ms": float(np.mean(b_ms)), "kernel_ms": kernel_ms,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_pos.numel() * 4),
+            # evaluated pairs/s alone rewards large leaves; these two do not
+            "time_to_solution_ms": ms_max / args.steps,
+            "within_cut_pairs_per_s": (within_cut_total * world / (ms_max / args.steps * 1e-3)) if within_cut_total else None,
+            "e2e": None if e2e_value is None else
+                   {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_pos.numel() * 4),
                     "d2h_bytes_per_step": int(h_acc.numel() * 4), "ms_per_step": e_ms_max / e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
@@ -370,12 +426,14 @@ def run_sweep(args):
     d_tgt = torch.from_numpy(tgt).cuda()
     out = torch.empty((cfg.n, 3), dtype=torch.float64, device="cuda")
     close = CLOSE_OVER_RCUT[cfg.kind] * r_cut
-    variants = [("fp32", "direct", {}), ("fp32", "poly", {})]
+    variants = [("fp32", "direct", {}), ("fp32", "fused", {}), ("fp32", "poly", {})]
     variants += [("fp32", "table", dict(table_nodes=n, table_level=2)) for n in (256, 512, 1024, 4096)]
     variants += [("fp32", "table", dict(table_nodes=512, table_level=lv)) for lv in (0, 1, 3)]
     variants += [("mixed", "direct", {}), ("mixed", "poly", {}), ("mixed", "table", dict(table_nodes=512, table_level=2))]
     variants += [("fp64", "direct", {}), ("fp64", "table", dict(table_nodes=512, table_level=4)),
-                 ("fp64", "table", dict(table_nodes=4096, table_level=3))]
+                 ("fp64", "table", dict(table_nodes=512, table_level=4, table_layout="coef")),
+                 ("fp64", "table", dict(table_nodes=4096, table_level=3)),
+                 ("fp64", "table", dict(table_nodes=4096, table_level=3, table_layout="coef"))]
     peak32 = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9
     print(f"# sweep on {cfg.name}: N = {cfg.n}, N_PM = {cfg.n_pm}, close_pair_radius = {close / r_cut:g} r_cut, "
           f"oracle on {len(tgt)} sampled targets (rms |a| = {rms:.4g}, {in_cut_per_particle:.0f} in-cut pairs per particle)\n")
@@ -396,10 +454,50 @@ def run_sweep(args):
             err = float(np.sqrt(((a - ref) ** 2).sum(axis=1)).max() / rms)
             ms = min(ks)
             rate = st["pairs_evaluated"] / (ms * 1e-3)
-            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]"
+            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]" + (" coef" if extra.get("table_layout") == "coef" else "")
             print(f"| {maxleaf} | {prec} | {gname} | {st['pairs_evaluated']:.4g} | {ms:.2f} | {rate:.3e} | "
                   f"{in_cut_per_particle * cfg.n / (ms * 1e-3):.3e} | {rate * PAPER_FLOPS_PER_PAIR / 1e12:.1f} | "
                   f"{100 * rate * PAPER_FLOPS_PER_PAIR / peak32:.1f} | {err:.2e} |", flush=True)
+    return 0
+
+
+def run_streams_study(args):
+    """a10 ("concurrency management"): the same step with target-leaf batches on 1, 2 and 4 CUDA streams:
+    P2P kernel time (CUDA events around all batches), whole device-resident step, and the host-buffer step."""
+    import torch
+    from paper_2107_14008_b200 import binding as B
+    cfg = workloads.CONFIGS[args.config]
+    pos, _ = workloads.make(cfg)
+    pos32 = pos.astype(np.float32)
+    del pos
+    d_pos = torch.from_numpy(pos32).cuda()
+    h_pos = torch.from_numpy(pos32).pin_memory()
+    d_acc = torch.empty((cfg.n, 3), dtype=torch.float32, device="cuda")
+    h_acc = torch.empty((cfg.n, 3), dtype=torch.float32).pin_memory()
+    stream = torch.cuda.current_stream()
+    print(f"# streams study on {cfg.name}: N = {cfg.n}, MAXLEAF = {cfg.maxleaf}, precision {args.precision}, g {args.g_mode}; "
+          f"median of {args.steps} steps after {args.warmup} warm-ups\n")
+    print("| n_streams | kernel ms | build ms | device-resident step ms | host-buffer step ms |")
+    print("|---|---|---|---|---|")
+    for ns in (1, 2, 4, 8):
+        with B.Photons(**headline_params(cfg, precision=args.precision, g_mode=args.g_mode, n_streams=ns)) as ph:
+            ph.set_stream(stream)
+            res = {}
+            for name, src, dst in (("dev", d_pos, d_acc), ("host", h_pos, h_acc)):
+                ks, bs, ts = [], [], []
+                for it in range(args.warmup + args.steps):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    ph.set_particles(src, None, stream=stream.cuda_stream)
+                    ph.build_leaves()
+                    st = ph.short_range_acc(dst)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    if it >= args.warmup:
+                        ks.append(st["kernel_ms"]); bs.append(st["build_ms"]); ts.append(e0.elapsed_time(e1))
+                res[name] = (float(np.median(ks)), float(np.median(bs)), float(np.median(ts)))
+        print(f"| {ns} | {res['dev'][0]:.2f} | {res['dev'][1]:.2f} | {res['dev'][2]:.2f} | {res['host'][2]:.2f} |", flush=True)
     return 0
 
 
@@ -451,11 +549,19 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=sorted(workloads.CONFIGS))
     ap.add_argument("--precision", default="fp32", choices=["fp32", "mixed", "fp64"])
-    ap.add_argument("--g-mode", dest="g_mode", default="poly", choices=["poly", "table", "direct"])
+    ap.add_argument("--g-mode", dest="g_mode", default="poly", choices=["poly", "table", "direct", "fused"])
+    ap.add_argument("--table-nodes", type=int, default=512)
+    ap.add_argument("--table-level", type=int, default=2)
+    ap.add_argument("--table-layout", default="paper", choices=["paper", "coef"])
+    ap.add_argument("--softening-over-rcut", type=float, default=0.0)
+    ap.add_argument("--warps-per-leaf", type=int, default=0)
+    ap.add_argument("--leaf-order", type=int, default=0, choices=[0, 1])
     ap.add_argument("--maxleaf", type=int, default=0)
     ap.add_argument("--streams", type=int, default=1)
     ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (ncu captures)")
+    ap.add_argument("--streams-study", action="store_true", help="kernel and step time for 1/2/4 streams (a10)")
     ap.add_argument("--sweep", action="store_true", help="MAXLEAF x g-mode x precision table instead of the bench line")
     ap.add_argument("--table-study", action="store_true", help="Eq. 2: table size x Taylor level, fp32 and fp64")
     ap.add_argument("--sweep-targets", type=int, default=1000)
@@ -463,8 +569,10 @@ def main(argv=None):
     args = ap.parse_args(argv)
     if args.steps < 1 or args.warmup < 0:
         ap.error("--steps >= 1 and --warmup >= 0")
-    if args.precision == "fp64" and args.g_mode == "poly":
-        args.g_mode = "direct"
+    if args.precision == "fp64" and args.g_mode in ("poly", "fused"):
+        args.g_mode = "direct"           # POLY and FUSED are fp32 approximations
+    if args.streams_study:
+        return run_streams_study(args)
     if args.sweep:
         return run_sweep(args)
     if args.table_study:

@@ -57,8 +57,11 @@ enum {
 enum {
     PHOTONS_G_DIRECT = 0, /* erfc/exp special functions per pair (what §3.3 L121 calls expensive) */
     PHOTONS_G_TABLE = 1,  /* Eq. 2 (L127-L143): table {T_i, E_i} in shared memory + Taylor terms T[0..level] */
-    PHOTONS_G_POLY = 2    /* no table, no special function: g/r^3 = 1/r^3 - Q(s)/(2 r_s)^3 with
+    PHOTONS_G_POLY = 2,   /* no table, no special function: g/r^3 = 1/r^3 - Q(s)/(2 r_s)^3 with
                              s = (r/2r_s)^2 and Q an FMA-pipe polynomial (fp32 paths only) */
+    PHOTONS_G_FUSED = 3   /* Eq. 1 evaluated directly per pair by a hand-fused routine instead of the stock erfcf/expf
+                             of G_DIRECT: g = exp(-x^2) H(x), the Gaussian by one ex2.approx (XU pipe), H = erfcx(x) +
+                             2x/sqrt(pi) by a polynomial of degree poly_degree (fp32 paths only) */
 };
 
 /* what the interpolation table holds per node (PHOTONS_G_TABLE) */
@@ -78,7 +81,7 @@ typedef struct {
     int n_pm;                 /* PM mesh cells per side (L33); must give r_cut < boxsize/2 */
     double rs_over_cell;      /* split radius in cells: 1.2 (L33) */
     double rcut_over_rs;      /* cut-off in r_s: 6.0 (north_star; the table spans x = r/2r_s in [0,3], L143);
-                                 must be <= 6 for g_mode TABLE and POLY (their range), any value for DIRECT */
+                                 must be <= 6 for g_mode TABLE, POLY and FUSED (their range), any value for DIRECT */
     double G;                 /* gravitational constant */
     int maxleaf;              /* MAXLEAF (L35): 16, 32, 64 or 128 */
     int precision;            /* PHOTONS_FP64 / FP32 / MIXED */
@@ -88,8 +91,10 @@ typedef struct {
                                  PHOTONS_FP64, 0..3 with FP32 / MIXED (T[2] already sits on the fp32 floor) */
     int n_streams;            /* >= 1: target-leaf batches are issued round-robin over this many CUDA streams */
     int device;               /* CUDA device ordinal */
-    double close_pair_radius; /* fp32/mixed paths: pairs with 0 < r < this are evaluated in fp64 inside the
-                                 kernel (A12); 0 = off.  Ignored by PHOTONS_FP64. */
+    double close_pair_radius; /* fp32/mixed paths, exact path (A12): a staged run of sources whose fp32 partial
+                                 acceleration on a target exceeds max|G m| / close_pair_radius^2 - what one pair at this
+                                 separation gives - is re-evaluated in fp64 for that target inside the kernel; 0 = off.
+                                 Ignored by PHOTONS_FP64. */
     int chunk_max;            /* largest number of source particle slots staged per shared-memory stage;
                                  0 = default (128); multiple of maxleaf, <= 256 */
     int warps_per_leaf;       /* warps of the CTA that owns one target leaf; they split its source list.
@@ -97,7 +102,8 @@ typedef struct {
     int targets_per_lane;     /* fp32/mixed kernels: targets a lane keeps in registers, 1, 2 or 4 (the warp then splits
                                  into 32 T / maxleaf groups that take alternate source pairs); 0 = default.
                                  Available: maxleaf 16: 1, 2; 32: 1, 2; 64: 2; 128: 4 */
-    int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12) */
+    int poly_degree;          /* POLY: degree of Q in the mapped variable, 10..14; 0 = default (12).
+                                 FUSED: degree of H, 9..11; 0 = default (10) */
     int periodic;             /* 1 = periodic cube of side boxsize, minimum image (default; north_star);
                                  0 = isolated boundaries: no images, positions are not wrapped,
                                  boxsize only sets r_s = rs_over_cell * boxsize / n_pm */
@@ -105,6 +111,9 @@ typedef struct {
                                  taken at r_eps = sqrt(r^2 + eps^2), a_i += G m_j d_ij g(r_eps) / r_eps^3 for pairs with
                                  0 < r and r_eps < r_cut.  0 = none (default; north_star's formula) */
     int table_layout;         /* TABLE: PHOTONS_TABLE_PAPER (default) or PHOTONS_TABLE_COEF */
+    int leaf_order;           /* order in which CTAs take the target leaves: 0 = longest source list first (default; shortens
+                                 the tail of clustered loads), 1 = ORB order (neighbouring leaves run together: their
+                                 source leaves are shared in L2) */
 } photons_params;
 
 typedef struct {
@@ -185,6 +194,10 @@ int photons_peak_probe(int device, int kind, double* out);
  * NULL): largest |approximation - g| over 0 <= r <= r_cut in exact arithmetic.  Errors: EINVAL (degree outside
  * 1..20, rcut_over_rs outside (0, 6], null coeffs). */
 int photons_poly_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g);
+
+/* Host-only: the polynomial behind PHOTONS_G_FUSED.  With x = r/2r_s, x_cut = rcut_over_rs/2 and t = 2 x/x_cut - 1 the
+ * kernels use g(r) ~= exp(-x^2) * sum_k coeffs[k] t^k.  Arguments, output and errors as photons_poly_fit. */
+int photons_fused_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g);
 
 /* Message of the last failing call on ctx; valid until the next call on ctx. */
 const char* photons_last_error(const photons_ctx* ctx);

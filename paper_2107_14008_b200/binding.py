@@ -16,20 +16,20 @@ LIB_PATH = os.path.join(_HERE, "libphotons.so")
 
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENODEVICE, EBOX, ENONFINITE = range(8)
 FP64, FP32, MIXED = 0, 1, 2
-G_DIRECT, G_TABLE, G_POLY = 0, 1, 2
+G_DIRECT, G_TABLE, G_POLY, G_FUSED = 0, 1, 2, 3
 TABLE_PAPER, TABLE_COEF = 0, 1
 MEM_HOST, MEM_DEVICE = 0, 1
 DTYPE_F64, DTYPE_F32 = 0, 1
 
 PRECISIONS = {"fp64": FP64, "fp32": FP32, "mixed": MIXED}
-G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY}
+G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY, "fused": G_FUSED}
 TABLE_LAYOUTS = {"paper": TABLE_PAPER, "coef": TABLE_COEF}
 ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX", "ENONFINITE"]
 
 EXPORTS = [
     "photons_default_params", "photons_create", "photons_set_stream", "photons_set_particles", "photons_build_leaves",
     "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
-    "photons_peak_probe", "photons_poly_fit", "photons_last_error", "photons_destroy",
+    "photons_peak_probe", "photons_poly_fit", "photons_fused_fit", "photons_last_error", "photons_destroy",
 ]
 
 
@@ -41,7 +41,7 @@ class Params(ctypes.Structure):
         ("table_level", ctypes.c_int), ("n_streams", ctypes.c_int), ("device", ctypes.c_int),
         ("close_pair_radius", ctypes.c_double), ("chunk_max", ctypes.c_int), ("warps_per_leaf", ctypes.c_int),
         ("targets_per_lane", ctypes.c_int), ("poly_degree", ctypes.c_int), ("periodic", ctypes.c_int),
-        ("softening", ctypes.c_double), ("table_layout", ctypes.c_int),
+        ("softening", ctypes.c_double), ("table_layout", ctypes.c_int), ("leaf_order", ctypes.c_int),
     ]
 
 
@@ -98,6 +98,8 @@ def load():
     lib.photons_peak_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.photons_poly_fit.restype = ci
     lib.photons_poly_fit.argtypes = [ci, ctypes.c_double, vp, ctypes.POINTER(ctypes.c_double)]
+    lib.photons_fused_fit.restype = ci
+    lib.photons_fused_fit.argtypes = [ci, ctypes.c_double, vp, ctypes.POINTER(ctypes.c_double)]
     lib.photons_last_error.restype = ctypes.c_char_p
     lib.photons_last_error.argtypes = [vp]
     lib.photons_destroy.restype = None
@@ -260,6 +262,16 @@ def poly_fit(degree: int, rcut_over_rs: float = 6.0):
     rc = load().photons_poly_fit(degree, float(rcut_over_rs), coeffs.ctypes.data, ctypes.byref(err))
     if rc != OK:
         raise PhotonsError(rc, "poly_fit: bad argument")
+    return coeffs, err.value
+
+
+def fused_fit(degree: int, rcut_over_rs: float = 6.0):
+    """(coeffs[degree+1] lowest power first, max |g_fused - g|) of the PHOTONS_G_FUSED polynomial; host only."""
+    coeffs = np.empty(degree + 1, dtype=np.float64)
+    err = ctypes.c_double()
+    rc = load().photons_fused_fit(degree, float(rcut_over_rs), coeffs.ctypes.data, ctypes.byref(err))
+    if rc != OK:
+        raise PhotonsError(rc, "fused_fit: bad argument")
     return coeffs, err.value
 
 

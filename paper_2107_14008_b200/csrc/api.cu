@@ -129,6 +129,7 @@ void photons_default_params(photons_params* p)
     p->periodic = 1;
     p->softening = 0.0;
     p->table_layout = PHOTONS_TABLE_PAPER;
+    p->leaf_order = 0;
 }
 
 static int create_fail(char* err_buf, int err_len, int code, const char* msg)
@@ -148,11 +149,11 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (p.maxleaf != 16 && p.maxleaf != 32 && p.maxleaf != 64 && p.maxleaf != 128)
         return create_fail(err_buf, err_len, PHOTONS_EINVAL, "maxleaf must be 16, 32, 64 or 128");
     if (p.precision < PHOTONS_FP64 || p.precision > PHOTONS_MIXED) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "bad precision");
-    if (p.g_mode < PHOTONS_G_DIRECT || p.g_mode > PHOTONS_G_POLY) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "bad g_mode");
-    if (p.g_mode == PHOTONS_G_POLY && p.precision == PHOTONS_FP64)
-        return create_fail(err_buf, err_len, PHOTONS_EINVAL, "g_mode POLY is an fp32 approximation; use DIRECT or TABLE with FP64");
+    if (p.g_mode < PHOTONS_G_DIRECT || p.g_mode > PHOTONS_G_FUSED) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "bad g_mode");
+    if ((p.g_mode == PHOTONS_G_POLY || p.g_mode == PHOTONS_G_FUSED) && p.precision == PHOTONS_FP64)
+        return create_fail(err_buf, err_len, PHOTONS_EINVAL, "g_mode POLY / FUSED are fp32 approximations; use DIRECT or TABLE with FP64");
     if (p.g_mode != PHOTONS_G_DIRECT && p.rcut_over_rs > 6.0)
-        return create_fail(err_buf, err_len, PHOTONS_EINVAL, "TABLE and POLY cover x = r/2r_s in [0,3]: rcut_over_rs must be <= 6");
+        return create_fail(err_buf, err_len, PHOTONS_EINVAL, "TABLE, POLY and FUSED cover x = r/2r_s in [0,3]: rcut_over_rs must be <= 6");
     if (p.g_mode == PHOTONS_G_TABLE) {
         if (p.table_nodes < 64 || p.table_nodes > 4096) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_nodes must be 64..4096");
         if (p.table_level < 0 || p.table_level > 4) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_level must be 0..4");
@@ -163,6 +164,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         if (p.table_layout == PHOTONS_TABLE_COEF && p.precision != PHOTONS_FP64)
             return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF is an option of the PHOTONS_FP64 path");
     }
+    if (p.leaf_order != 0 && p.leaf_order != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "leaf_order must be 0 or 1");
     if (p.n_streams < 1 || p.n_streams > 64) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "n_streams must be 1..64");
     if (p.close_pair_radius < 0 || !std::isfinite(p.close_pair_radius)) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be >= 0");
     if (p.chunk_max == 0) p.chunk_max = p.maxleaf > 128 ? p.maxleaf : 128;
@@ -177,8 +179,13 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         const bool ok = (m == 16 && (t == 1 || t == 2)) || (m == 32 && (t == 1 || t == 2)) || (m == 64 && t == 2) || (m == 128 && t == 4);
         if (!ok) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "targets_per_lane not available for this maxleaf");
     }
-    if (p.poly_degree == 0) p.poly_degree = 12;
-    if (p.poly_degree < 10 || p.poly_degree > 14) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "poly_degree must be 10..14");
+    if (p.g_mode == PHOTONS_G_FUSED) {
+        if (p.poly_degree == 0) p.poly_degree = 10;
+        if (p.poly_degree < 9 || p.poly_degree > 11) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "poly_degree must be 9..11 with g_mode FUSED");
+    } else {
+        if (p.poly_degree == 0) p.poly_degree = 12;
+        if (p.poly_degree < 10 || p.poly_degree > 14) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "poly_degree must be 10..14");
+    }
 
     const double r_s = p.rs_over_cell * p.boxsize / p.n_pm;
     const double r_cut = p.rcut_over_rs * r_s;
@@ -223,6 +230,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     if (!ok) rc = fail(c, PHOTONS_ECUDA, "stream/event creation failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == PHOTONS_OK && p.g_mode == PHOTONS_G_TABLE) rc = make_table(c);
     if (rc == PHOTONS_OK && p.g_mode == PHOTONS_G_POLY) rc = make_poly(c);
+    if (rc == PHOTONS_OK && p.g_mode == PHOTONS_G_FUSED) rc = make_fused(c);
     if (rc != PHOTONS_OK) {
         create_fail(err_buf, err_len, rc, c->err.c_str());
         photons_destroy(reinterpret_cast<photons_ctx*>(c));
@@ -288,6 +296,7 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     double m_max;
     memcpy(&m_max, &h_flags[1], sizeof m_max);
     const double gm_max = std::fabs(c->p.G) * m_max;
+    c->gm_max = gm_max;
     c->gmscale = gm_max > 0 && std::isfinite(gm_max) ? std::ldexp(1.0, (int)std::ceil(std::log2(gm_max))) : 1.0;
     c->n = n;
     return PHOTONS_OK;

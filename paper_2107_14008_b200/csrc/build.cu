@@ -629,6 +629,8 @@ int build_leaves_impl(Ctx* c)
         if (!tmp) return PHOTONS_ENOMEM;
         PH_CUDA_BUILD(cub::DeviceRadixSort::SortPairsDescending(tmp, sort_bytes, d_okeys, d_okeys2, d_ovals, c->d_order, (int)n_leaves, 0, 32, st));
     }
+    if (c->p.leaf_order == 1)      // ORB order: d_ovals is the identity
+        PH_CUDA_BUILD(cudaMemcpyAsync(c->d_order, d_ovals, sizeof(int) * n_leaves, cudaMemcpyDeviceToDevice, st));
     unsigned h_last = 0;
     PH_CUDA_BUILD(cudaMemcpyAsync(&h_last, d_okeys2, sizeof(unsigned), cudaMemcpyDeviceToHost, st));   // largest work
     PH_CUDA_BUILD(cudaStreamSynchronize(st));

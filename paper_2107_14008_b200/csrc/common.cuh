@@ -61,6 +61,7 @@ struct Ctx {
     // pscale (the power of two just below r_cut), G m by gmscale (the power of two >= max |G m|); sums are scaled back
     // in fp64 by gmscale / pscale^2 when they are stored
     double pscale = 1.0, gmscale = 1.0;
+    double gm_max = 0.0;                 // max |G m_j| of the current particle set
     int sm_count = 0;
     std::vector<const void*> smem_opted;  // kernels whose dynamic shared-memory limit has been raised already
     std::vector<cudaStream_t> streams;   // [0] = main stream (the caller's after photons_set_stream)
@@ -95,6 +96,9 @@ struct Ctx {
     int poly_deg = 0;
     float poly_c[POLY_MAX_DEG + 1]{};   // Q(s)/(2 r_s)^3 as a polynomial in t = 2 s/s_max - 1, Horner order
     double poly_err = 0;                // max |g_poly - g| over [0, x_cut] in exact arithmetic
+    int fused_deg = 0;
+    float fused_c[POLY_MAX_DEG + 1]{};  // H(x) = erfcx(x) + 2x/sqrt(pi) as a polynomial in t = 2 x/x_cut - 1, Horner order
+    double fused_err = 0;               // max |exp(-x^2) H_poly(x) - g| over [0, x_cut] in exact arithmetic
 
     DevBuf ws[WS_COUNT];
 
@@ -124,6 +128,7 @@ void free_leaves(Ctx* c);
 // gfunc.cu
 int make_table(Ctx* c);
 int make_poly(Ctx* c);
+int make_fused(Ctx* c);
 // p2p_fp64.cu / p2p_fp32.cu: enqueue the kernel for target leaves order[first .. first+count) on a stream;
 // out = device buffer in caller order (n x 3, fp64 or fp32 as out_f32 says)
 int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool out_f32, cudaStream_t st);

@@ -97,24 +97,20 @@ static void lstsq(std::vector<long double>& A, std::vector<long double>& b, int 
     }
 }
 
-// mono[k] = coefficient of t^k (k = 0..deg), t = 2 s/s_max - 1, s_max = (rcut_over_rs / 2)^2; returns the
-// largest |g_poly - g| over [0, x_cut] in exact arithmetic
-static long double fit_poly(int deg, long double rcut_over_rs, std::vector<long double>& mono)
+// Weighted minimax fit on t in [-1, 1] in the Chebyshev basis: Lawson's iteration (repeated weighted least squares,
+// weights multiplied by the residual) on a Chebyshev-distributed sample, in long double; one degree cheaper than plain
+// Chebyshev interpolation at equal accuracy.  mono[k] = coefficient of t^k (k = 0..deg).
+// `target` supplies f(t), the function to fit, and w(t), the weight of the residual.
+template <typename Target>
+static void lawson_fit(int deg, const Target& target, std::vector<long double>& mono)
 {
     const int N = deg + 1;
-    const long double xcut = 0.5L * rcut_over_rs;
-    const long double smax = xcut * xcut;
-    // Weighted minimax fit of Q on [0, s_max] in the Chebyshev basis of t = 2 s/s_max - 1: what matters is the
-    // error of g = 1 - x^3 Q, so the residual carries the weight s^(3/2).  Lawson's iteration (repeated
-    // weighted least squares, weights multiplied by the residual) on a Chebyshev-distributed sample; one
-    // degree cheaper than plain Chebyshev interpolation at equal accuracy in g.
     const int M = 48 * N;
     std::vector<long double> tt(M), qq(M), wg(M), lw(M, 1.0L), cheb(N, 0.0L);
     for (int i = 0; i < M; ++i) {
         tt[i] = cosl(PI_L * (i + 0.5L) / M);
-        const long double s = 0.5L * smax * (tt[i] + 1.0L);
-        qq[i] = Q_of_s(s);
-        wg[i] = s * sqrtl(s);
+        qq[i] = target.f(tt[i]);
+        wg[i] = target.w(tt[i]);
     }
     std::vector<long double> V((size_t)M * N);
     for (int i = 0; i < M; ++i) {
@@ -156,7 +152,22 @@ static long double fit_poly(int deg, long double rcut_over_rs, std::vector<long 
         Tkm1 = Tk;
         Tk = Tkp1;
     }
-    // truncation error of the polynomial, expressed as an error of g:  |x^3 (P - Q)|
+}
+
+// POLY: Q on [0, s_max] in t = 2 s/s_max - 1, s_max = (rcut_over_rs / 2)^2.  What matters is the error of g = 1 - x^3 Q,
+// so the residual carries the weight s^(3/2).  Returns the largest |g_poly - g| over [0, x_cut] in exact arithmetic.
+struct PolyTarget {
+    long double smax;
+    long double s(long double t) const { return 0.5L * smax * (t + 1.0L); }
+    long double f(long double t) const { return Q_of_s(s(t)); }
+    long double w(long double t) const { return s(t) * sqrtl(s(t)); }
+};
+
+static long double fit_poly(int deg, long double rcut_over_rs, std::vector<long double>& mono)
+{
+    const long double xcut = 0.5L * rcut_over_rs;
+    const long double smax = xcut * xcut;
+    lawson_fit(deg, PolyTarget{smax}, mono);
     long double worst = 0;
     for (int i = 0; i <= 4000; ++i) {
         const long double s = smax * i / 4000.0L;
@@ -167,6 +178,44 @@ static long double fit_poly(int deg, long double rcut_over_rs, std::vector<long 
         if (e > worst) worst = e;
     }
     return worst;
+}
+
+// FUSED: Eq. 1 factorised as g(x) = exp(-x^2) H(x), H(x) = erfcx(x) + 2 x / sqrt(pi) (erfcx = exp(x^2) erfc):
+// H is smooth and of order one on [0, x_cut] (H(0) = 1, H' = 2 x erfcx), so a polynomial in t = 2 x/x_cut - 1 of
+// degree ~10 reproduces it; the residual carries the weight exp(-x^2), i.e. the fit is minimax in g.
+static long double H_of_x(long double x) { return erfcl(x) * expl(x * x) + 2.0L * x / sqrtl(PI_L); }
+
+struct FusedTarget {
+    long double xcut;
+    long double x(long double t) const { return 0.5L * xcut * (t + 1.0L); }
+    long double f(long double t) const { return H_of_x(x(t)); }
+    long double w(long double t) const { return expl(-x(t) * x(t)); }
+};
+
+static long double fit_fused(int deg, long double rcut_over_rs, std::vector<long double>& mono)
+{
+    const long double xcut = 0.5L * rcut_over_rs;
+    lawson_fit(deg, FusedTarget{xcut}, mono);
+    long double worst = 0;
+    for (int i = 0; i <= 4000; ++i) {
+        const long double x = xcut * i / 4000.0L;
+        const long double t = 2.0L * x / xcut - 1.0L;
+        long double p = 0;
+        for (int k = deg; k >= 0; --k) p = p * t + mono[k];
+        const long double e = fabsl(expl(-x * x) * (p - H_of_x(x)));
+        if (e > worst) worst = e;
+    }
+    return worst;
+}
+
+int make_fused(Ctx* c)
+{
+    const int deg = c->p.poly_degree;
+    std::vector<long double> mono;
+    c->fused_err = (double)fit_fused(deg, c->p.rcut_over_rs, mono);
+    c->fused_deg = deg;
+    for (int i = 0; i <= deg; ++i) c->fused_c[i] = (float)mono[deg - i];     // Horner order (highest degree first)
+    return PHOTONS_OK;
 }
 
 int make_poly(Ctx* c)
@@ -185,7 +234,17 @@ int make_poly(Ctx* c)
 
 }  // namespace photons
 
-// Host-only hook (no device needed): the fitted polynomial itself, for checks against an independent g.
+// Host-only hooks (no device needed): the fitted polynomials themselves, for checks against an independent g.
+extern "C" int photons_fused_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g)
+{
+    if (degree < 1 || degree > photons::POLY_MAX_DEG || !(rcut_over_rs > 0) || rcut_over_rs > 6.0 || !coeffs) return PHOTONS_EINVAL;
+    std::vector<long double> mono;
+    const long double e = photons::fit_fused(degree, rcut_over_rs, mono);
+    for (int k = 0; k <= degree; ++k) coeffs[k] = (double)mono[k];
+    if (max_err_g) *max_err_g = (double)e;
+    return PHOTONS_OK;
+}
+
 extern "C" int photons_poly_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g)
 {
     if (degree < 1 || degree > photons::POLY_MAX_DEG || !(rcut_over_rs > 0) || rcut_over_rs > 6.0 || !coeffs) return PHOTONS_EINVAL;

@@ -23,7 +23,7 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     while ((1 << a.log2m) < a.maxleaf) ++a.log2m;
     a.chunk_max = c->p.chunk_max; a.mixed = c->p.precision == PHOTONS_MIXED;
     // kernel units: lengths / pscale, G m / gmscale (common.cuh); everything the pair core touches is O(1)
-    const double ps = c->pscale, ips = 1.0 / c->pscale;
+    const double ips = 1.0 / c->pscale;
     const double Ls = c->p.boxsize * ips, rs = c->r_s * ips, rcut = c->r_cut * ips;
     a.inv_pscale = ips;
     a.oscale = c->gmscale * ips * ips;
@@ -33,21 +33,20 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     const double eps = c->p.softening * ips;
     a.r2add = std::fmax(R2_FLOOR, (float)(eps * eps));
     a.eps2_d = c->p.softening * c->p.softening;
-    a.rclose2 = (float)(c->p.close_pair_radius * ips * c->p.close_pair_radius * ips);
-    if (!(a.rclose2 > 2.0f * a.r2add)) a.rclose2 = 0.f;      // nothing left to redo exactly inside the softening core
-    a.Ld = c->p.boxsize; a.inv2rs_d = 1.0 / (2.0 * c->r_s);
-    // the fast path clamps at the fp32 value of r_close^2; the exact path uses the same radius (caller units)
-    a.rclose_d = std::sqrt((double)a.rclose2) * ps;
-    a.wclose_d = 0.0;
-    if (a.rclose_d > 0) {
-        const double x = a.rclose_d * a.inv2rs_d;
-        const double g = std::erfc(x) + 1.1283791670955125739 * x * std::exp(-x * x);
-        a.wclose_d = g / (a.rclose_d * a.rclose_d * a.rclose_d);
+    a.Ld = c->p.boxsize; a.inv2rs_d = 1.0 / (2.0 * c->r_s); a.rcut2_d = c->r_cut * c->r_cut;
+    // exact path trigger: |fp32 partial of a run| > max|G m| / r_close^2 (one pair at r_close), in kernel units
+    a.pth2 = 0.f;
+    if (c->p.close_pair_radius > 0) {
+        const double rc = c->p.close_pair_radius * ips;
+        const double pth = (c->gm_max / c->gmscale) / (rc * rc);
+        a.pth2 = (float)std::fmin(pth * pth, 1e37);
     }
     a.inv2rs = (float)(1.0 / (2.0 * rs));
     const double smax = 0.25 * c->p.rcut_over_rs * c->p.rcut_over_rs;
     a.tk = (float)(2.0 / (smax * 4.0 * rs * rs));
-    for (int i = 0; i <= POLY_MAX_DEG; ++i) a.pc[i] = c->poly_c[i];
+    for (int i = 0; i <= POLY_MAX_DEG; ++i) a.pc[i] = c->p.g_mode == PHOTONS_G_FUSED ? c->fused_c[i] : c->poly_c[i];
+    a.ek = (float)(-1.4426950408889634 / (4.0 * rs * rs));          // exp(-x^2) = 2^(-x^2 log2 e), x^2 = r^2 / 4 r_s^2
+    a.tmap = (float)(2.0 / (0.5 * c->p.rcut_over_rs));
     a.tn = c->table.n;
     a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
     a.uk = a.tn ? (float)(a.tn / 3.0 / (2.0 * rs)) : 0.f;
@@ -63,6 +62,7 @@ int launch_p2p_fp32(Ctx* c, long long first, long long count, void* out, bool ou
     switch (c->p.g_mode) {
         case PHOTONS_G_POLY: return launch_p32_poly(c, a, count, st);
         case PHOTONS_G_TABLE: return launch_p32_table(c, a, count, st);
+        case PHOTONS_G_FUSED: return launch_p32_fused(c, a, count, st);
         default: return launch_p32_direct(c, a, count, st);
     }
 }

@@ -5,7 +5,7 @@ namespace photons {
 
 int launch_p32_direct(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
 {
-    return launch_p32_close<GM_DIRECT, 0>(c, a, count, st);
+    return launch_p32_shape<GM_DIRECT, 0>(c, a, count, st);
 }
 
 }  // namespace photons

@@ -9,7 +9,9 @@
 //   pair core      two sources per lane per step in packed fp32 (add/mul/fma.rn.f32x2 -> FADD2/FMUL2/FFMA2),
 //                  one MUFU.RSQ per pair; sources are read as two broadcast LDS.128 per step
 //   accumulation   fp32 per staged run, flushed into fp64 per-lane sums (two-level, A12)
-//   close pairs    optional: pairs inside close_pair_radius are clamped in the fast path and redone in fp64
+//   exact path     optional (close_pair_radius > 0): a staged run whose fp32 partial acceleration on a target exceeds
+//                  what one pair at close_pair_radius would give is re-evaluated in fp64 from the exact coordinates
+//                  for that target (nothing per pair in the fast path: three compares per run)
 //   units          lengths in units of Ctx::pscale (a power of two near r_cut), G m in units of Ctx::gmscale (a power
 //                  of two >= max |G m|): exact rescalings that keep every fp32 intermediate in range whatever the
 //                  caller's units are; the fp64 sums are scaled back when they are stored
@@ -36,7 +38,7 @@ constexpr float MAGIC = 12582912.0f;     // 1.5 * 2^23: float -> nearest-integer
 
 struct P32Args {
     const float* p32;          // n_slots/2 x {x0 x1 y0 y1 z0 z1 Gm0 Gm1}
-    const double4* p64;        // n_slots x {x, y, z, G m}: exact coordinates for the close-pair path
+    const double4* p64;        // n_slots x {x, y, z, G m}: exact coordinates for the exact path
     const double* ctr;         // n_leaves x 3: origin of each leaf's offsets (MIXED), else unused
     const int* slot_src;
     const long long* chunk_ptr;
@@ -45,13 +47,15 @@ struct P32Args {
     long long first;
     int maxleaf, log2m, chunk_max, mixed;
     float Lh, Ll, invL;        // box length in kernel units as an unevaluated sum of two floats (exact image shifts)
-    float rcut2, rclose2;      // kernel units; both compared with r^2 + r2add
+    float rcut2;               // kernel units; compared with r^2 + r2add
+    float pth2;                // exact path: square of the run-partial acceleration that triggers it (kernel units); 0 = off
     float r2add;               // max(R2_FLOOR, eps^2): start value of every r^2 chain
-    double Ld, inv2rs_d, rclose_d, wclose_d, eps2_d;   // caller units (close pairs): g(r_close)/r_close^3 in fp64
+    double Ld, inv2rs_d, rcut2_d, eps2_d;   // caller units, for the exact path
     double inv_pscale;         // 1 / Ctx::pscale
     double oscale, inv_oscale; // kernel-unit sums -> caller units: gmscale / pscale^2
     float inv2rs;              // 1 / 2 r_s (kernel units)
     float tk;                  // POLY: t = r2 * tk - 1
+    float ek, tmap;            // FUSED: exp(-x^2) = ex2(r2 * ek); t = x * tmap - 1 maps [0, x_cut] to [-1, 1]
     float pc[POLY_MAX_DEG + 1];
     float uk, h, umax;         // TABLE: u = r * uk in node units, h = 3/n, umax = last node
     int tn;
@@ -66,6 +70,13 @@ __device__ __forceinline__ float rsq(float x)
 {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// one MUFU.EX2
+__device__ __forceinline__ float ex2(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
@@ -90,6 +101,21 @@ __device__ __forceinline__ float2 weight_poly(const P32Args& a, float2 r2, float
     const float2 idr2 = __fmul2_rn(idr, idr);
     const float2 u = __ffma2_rn(idr2, idr, f2(-q.x, -q.y));          // 1/r^3 - Q(s)/(2 r_s)^3
     return __fmul2_rn(u, gm);
+}
+
+template <int DEG>
+__device__ __forceinline__ float2 weight_fused(const P32Args& a, float2 r2, float2 gm)
+{
+    const float2 idr = f2(rsq(r2.x), rsq(r2.y));
+    const float2 x = __fmul2_rn(__fmul2_rn(r2, idr), dup(a.inv2rs));
+    const float2 t = __ffma2_rn(x, dup(a.tmap), dup(-1.0f));
+    const float2 y = __fmul2_rn(r2, dup(a.ek));
+    const float2 e = f2(ex2(y.x), ex2(y.y));
+    float2 q = dup(a.pc[0]);
+#pragma unroll
+    for (int k = 1; k <= DEG; ++k) q = __ffma2_rn(q, t, dup(a.pc[k]));
+    const float2 idr2 = __fmul2_rn(idr, idr);
+    return __fmul2_rn(__fmul2_rn(q, e), __fmul2_rn(idr2, __fmul2_rn(idr, gm)));
 }
 
 template <int LEVEL>
@@ -136,7 +162,7 @@ __device__ __forceinline__ float weight_direct1(const P32Args& a, float r2, floa
     return gm * g * (idr * idr * idr);
 }
 
-enum { GM_POLY = 0, GM_TABLE = 1, GM_DIRECT = 2 };
+enum { GM_POLY = 0, GM_TABLE = 1, GM_DIRECT = 2, GM_FUSED = 3 };
 
 template <int GKIND, int GPAR>
 __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, float2 r2, float2 gm)
@@ -144,6 +170,7 @@ __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, f
     float2 w;
     if (GKIND == GM_POLY) w = weight_poly<GPAR>(a, r2, gm);
     else if (GKIND == GM_TABLE) w = weight_table<GPAR>(a, tab, r2, gm);
+    else if (GKIND == GM_FUSED) w = weight_fused<GPAR>(a, r2, gm);
     else w = f2(weight_direct1(a, r2.x, gm.x), weight_direct1(a, r2.y, gm.y));
     // the cut (A8) and, with it, everything the approximations do outside their range
     return f2(r2.x < a.rcut2 ? w.x : 0.f, r2.y < a.rcut2 ? w.y : 0.f);
@@ -155,7 +182,7 @@ __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, f
 // kc: the loop constants (polynomial coefficients, tk, r_cut^2) as one local object
 struct LoopConst {
     float pc[POLY_MAX_DEG + 1];
-    float tk, rcut2, r2add;
+    float tk, rcut2, r2add, ek, tmap, inv2rs;
 };
 
 template <int GKIND, int GPAR, int NCH>
@@ -182,29 +209,70 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
             const float2 v = __fmul2_rn(u, gm[c]);
             w[c] = f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f);
         }
+    } else if (GKIND == GM_FUSED) {
+        // Eq. 1 evaluated directly, hand-fused: g = exp(-x^2) H(x) with H = erfcx(x) + 2x/sqrt(pi), smooth on [0, 3]:
+        // one MUFU.EX2 for the Gaussian (its argument straight from r^2) and a degree-GPAR polynomial for H on the
+        // FMA pipe, against the stock erfcf + expf of GM_DIRECT (5 MUFU + 1 FRND + ~55 FP32 instructions per pair)
+        float2 idr[NCH], t[NCH], q[NCH], e[NCH];
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            idr[c] = f2(rsq(r2[c].x), rsq(r2[c].y));
+            const float2 x = __fmul2_rn(__fmul2_rn(r2[c], idr[c]), dup(kc.inv2rs));
+            t[c] = __ffma2_rn(x, dup(kc.tmap), dup(-1.0f));
+            const float2 y = __fmul2_rn(r2[c], dup(kc.ek));
+            e[c] = f2(ex2(y.x), ex2(y.y));
+            q[c] = __ffma2_rn(dup(kc.pc[0]), t[c], dup(kc.pc[1]));
+        }
+#pragma unroll
+        for (int k = 2; k <= GPAR; ++k) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) q[c] = __ffma2_rn(q[c], t[c], dup(kc.pc[k]));
+        }
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
+            const float2 v = __fmul2_rn(__fmul2_rn(q[c], e[c]), __fmul2_rn(idr2, __fmul2_rn(idr[c], gm[c])));
+            w[c] = f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f);
+        }
     } else {
 #pragma unroll
         for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR>(a, tab, r2[c], gm[c]);
     }
 }
 
-// smallest r^2 seen so far, self / coincident pairs (r^2 == r2add exactly) excluded: as unsigned integers
-// the bit patterns of positive floats keep their order, and subtracting base = bits(r2add) + 1 wraps the
-// excluded value to the top (two ALU-pipe integer ops per pair instead of a compare, a select and a min)
-__device__ __forceinline__ unsigned close_key(float r2, unsigned base) { return (unsigned)__float_as_int(r2) - base; }
-
-// exact weight difference for a close pair, fp64: G m_j [g(r)/r^3 - g(r_c)/r_c^3]
-static __device__ __noinline__ double close_pair_weight(double r2, double gm, double inv2rs, double wclose)
+// Exact path (A12): one target against one staged run of sources, in fp64 from the exact coordinates with
+// the library's erfc / exp — the oracle's arithmetic.  Sources j = first, first + step, ... < ns of the run at e.x.
+// Returns the acceleration in caller units.
+static __device__ __noinline__ double3 exact_run(const P32Args& a, int tslot, uint2 e, int first, int step)
 {
-    const double r = sqrt(r2);
-    const double x = r * inv2rs;
-    const double g = erfc(x) + 1.1283791670955125739 * x * exp(-x * x);
-    return gm * (g / (r2 * r) - wclose);
+    const int ns = (int)(e.y & 0xffffu);
+    const bool per_pair = (e.y & ENTRY_PER_PAIR) != 0;
+    const double sx = a.Ld * ((int)((e.y >> 16) & 3u) - 1), sy = a.Ld * ((int)((e.y >> 18) & 3u) - 1), sz = a.Ld * ((int)((e.y >> 20) & 3u) - 1);
+    const double4 pi = a.p64[tslot];
+    double ax = 0, ay = 0, az = 0;
+    for (int j = first; j < ns; j += step) {
+        const double4 pj = a.p64[e.x + j];
+        double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        if (per_pair) {
+            dx -= a.Ld * rint(dx / a.Ld); dy -= a.Ld * rint(dy / a.Ld); dz -= a.Ld * rint(dz / a.Ld);
+        } else {
+            dx += sx; dy += sy; dz += sz;
+        }
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        const double r2e = r2 + a.eps2_d;
+        if (r2 > 0.0 && r2e < a.rcut2_d) {
+            const double r = sqrt(r2e);
+            const double x = r * a.inv2rs_d;
+            const double w = pj.w * (erfc(x) + 1.1283791670955125739 * x * exp(-x * x)) / (r2e * r);
+            ax += w * dx; ay += w * dy; az += w * dz;
+        }
+    }
+    return make_double3(ax, ay, az);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 
-template <int T, int HS, bool MIXED, int GKIND, int GPAR, bool CLOSE>
+template <int T, int HS, bool MIXED, int GKIND, int GPAR>
 __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -236,14 +304,14 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
     }
 
     LoopConst kc;
-    if (GKIND == GM_POLY) {
+    if (GKIND == GM_POLY || GKIND == GM_FUSED) {
 #pragma unroll
         for (int k = 0; k <= GPAR; ++k) kc.pc[k] = a.pc[k];
     }
+    kc.ek = a.ek; kc.tmap = a.tmap; kc.inv2rs = a.inv2rs;
     kc.tk = a.tk;
     kc.rcut2 = a.rcut2;
     kc.r2add = a.r2add;
-    const unsigned ckbase = (unsigned)__float_as_int(a.r2add) + 1u;
 
     // targets -> registers (Alg. 1 L99)
     float tx[T], ty[T], tz[T];
@@ -323,7 +391,6 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
         float px[T], py[T], pz[T];       // fp32 partial sums of this run (level 1 of the accumulation)
 #pragma unroll
         for (int t = 0; t < T; ++t) px[t] = py[t] = pz[t] = 0.f;
-        unsigned kmin = 0xffffffffu;     // close_key of the closest non-coincident pair of this run
 
         for (int b0 = 0; b0 < ns; b0 += blk) {
             // targets as seen from this block: d = (r_j + sadd) - q
@@ -363,7 +430,6 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                             dy = fmaf(-a.Ll, iy, fmaf(-a.Lh, iy, dy));
                             dz = fmaf(-a.Ll, iz, fmaf(-a.Lh, iz, dz));
                             float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.r2add)));
-                            if (CLOSE) { kmin = min(kmin, close_key(r2, ckbase)); r2 = fmaxf(r2, a.rclose2); }
                             const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
                         }
@@ -398,10 +464,6 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 #pragma unroll
                     for (int c = 0; c < NCH; ++c) {
                         r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(kc.r2add))));
-                        if (CLOSE) {
-                            kmin = min(kmin, min(close_key(r2[c].x, ckbase), close_key(r2[c].y, ckbase)));
-                            r2[c] = f2(fmaxf(r2[c].x, a.rclose2), fmaxf(r2[c].y, a.rclose2));
-                        }
                     }
                     weights<GKIND, GPAR, NCH>(a, kc, tab, r2, gm, w);
 #pragma unroll
@@ -427,36 +489,22 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
                 }
             }
         }
-        // level 2 of the accumulation: flush the run's fp32 partial sums into the fp64 sums
+        // Exact path: a run whose partial sum is larger than one pair at close_pair_radius would give holds a pair
+        // close enough for fp32 rounding (3 ulp of the rsqrt in 1/r^3) to show against the tolerance: redo the run
+        // in fp64 for this target and drop the fp32 partial.
+        if (a.pth2 > 0.f) {
 #pragma unroll
-        for (int t = 0; t < T; ++t) { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
-
-        if (CLOSE) {
-            // The fast path evaluated pairs inside r_close as if they sat at r_close.  Redo those pairs in
-            // fp64 from the exact coordinates.  Self pairs do not trigger the scan (close_key), so it runs
-            // only for runs that really hold a close pair.
-            if (__any_sync(0xffffffffu, kmin < close_key(a.rclose2, ckbase))) {
-#pragma unroll
-                for (int t = 0; t < T; ++t) {
-                    const double4 pi = a.p64[tslot[t]];
-                    for (int j = half; j < ns; j += pstep) {
-                        const double4 pj = a.p64[e.x + j];
-                        double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-                        if (per_pair) {
-                            dx -= a.Ld * rint(dx / a.Ld); dy -= a.Ld * rint(dy / a.Ld); dz -= a.Ld * rint(dz / a.Ld);
-                        } else {
-                            dx += a.Ld * sxi; dy += a.Ld * syi; dz += a.Ld * szi;
-                        }
-                        const double r2 = dx * dx + dy * dy + dz * dz;
-                        const double r2e = r2 + a.eps2_d;
-                        if (r2 > 0.0 && r2e < a.rclose_d * a.rclose_d) {
-                            const double w = close_pair_weight(r2e, pj.w, a.inv2rs_d, a.wclose_d) * a.inv_oscale;
-                            ax[t] += w * dx; ay[t] += w * dy; az[t] += w * dz;
-                        }
-                    }
+            for (int t = 0; t < T; ++t) {
+                if (fmaf(px[t], px[t], fmaf(py[t], py[t], pz[t] * pz[t])) > a.pth2) {
+                    const double3 x = exact_run(a, tslot[t], e, half, pstep);
+                    ax[t] += x.x * a.inv_oscale; ay[t] += x.y * a.inv_oscale; az[t] += x.z * a.inv_oscale;
+                    px[t] = py[t] = pz[t] = 0.f;
                 }
             }
         }
+        // level 2 of the accumulation: flush the run's fp32 partial sums into the fp64 sums
+#pragma unroll
+        for (int t = 0; t < T; ++t) { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
         __syncwarp();
         if (k + N_STAGES < n_my) issue(k + N_STAGES, batch, st);
         if (++st == N_STAGES) { st = 0; phase ^= 1u; }
@@ -508,7 +556,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32);
 size_t p32_smem_bytes(Ctx* c, int T);
 
-template <int GKIND, int GPAR, bool CLOSE>
+template <int GKIND, int GPAR>
 static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
 {
     const int W = c->p.warps_per_leaf;
@@ -517,7 +565,7 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     const size_t smem = p32_smem_bytes(c, T);
     void (*kern)(P32Args) = nullptr;
     const bool mixed = c->p.precision == PHOTONS_MIXED;
-#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR, CLOSE> : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR, CLOSE>)
+#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR> : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR>)
     switch (M * 8 + T) {   // (MAXLEAF, targets per lane) -> (T, lane groups)
         case 16 * 8 + 1: kern = PH_SHAPE(1, 2); break;
         case 16 * 8 + 2: kern = PH_SHAPE(2, 4); break;
@@ -535,17 +583,11 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     return PHOTONS_OK;
 }
 
-template <int GKIND, int GPAR>
-static int launch_p32_close(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
-{
-    return a.rclose2 > 0.f ? launch_p32_shape<GKIND, GPAR, true>(c, a, count, st)
-                           : launch_p32_shape<GKIND, GPAR, false>(c, a, count, st);
-}
-
 int launch_p32_poly(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 template <int DEG>
 int launch_p32_poly_deg(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 int launch_p32_table(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 int launch_p32_direct(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
+int launch_p32_fused(Ctx* c, const P32Args& a, long long count, cudaStream_t st);
 
 }  // namespace photons

@@ -6,7 +6,7 @@ namespace photons {
 template <>
 int launch_p32_poly_deg<11>(Ctx* c, const P32Args& a, long long count, cudaStream_t st)
 {
-    return launch_p32_close<GM_POLY, 11>(c, a, count, st);
+    return launch_p32_shape<GM_POLY, 11>(c, a, count, st);
 }
 
 }  // namespace photons

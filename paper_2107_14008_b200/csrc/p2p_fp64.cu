@@ -15,7 +15,9 @@
 //         node with the node polynomials folded in when the table is built (Horner only: `level` DFMAs).  The paper
 //         tabulates two numbers per node "considering the suitable capacity of shared memory" (L143, 96 KB on V100);
 //         with 227 KB per SM on B200 the 5-column table of 512 nodes (20 KB) is the cheaper trade.
-//   - index by the magic-number add in fp64 (the low word of u + 1.5 * 2^52 is the nearest integer): no F2I/I2F.
+//   - index by the magic-number add in fp64 (the low word of u + 1.5 * 2^52 is the nearest integer): no F2I/I2F;
+//     u itself is never formed: fma(r, uk, MAGIC) and eps = fma(r, 1/2r_s, -x_i);
+//   - the cut compare on the integer pipe (bit patterns of positive doubles are ordered).
 #include "common.cuh"
 #include "pipeline.cuh"
 
@@ -62,29 +64,30 @@ __device__ __forceinline__ double rsqrt64(double x)
 
 // g(x) for NCH chains at once; r = r2 * idr is passed in
 template <int GMODE, int LEVEL, int NCH>
-__device__ __forceinline__ void g_eval(const P64Args& a, const double* __restrict__ tab, const double (&r)[NCH], double (&g)[NCH])
+__device__ __forceinline__ void g_eval(const P64Args& a, const double* __restrict__ tab, const double (&r)[NCH],
+                                       const bool (&incut)[NCH], double (&g)[NCH])
 {
     if constexpr (GMODE == G64_DIRECT) {
+        // the library's erfc + exp cost ~90 DP instructions: skip them for sources no lane of the warp has inside the cut
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) g[c] = g_direct64(r[c] * a.inv2rs);
+        for (int c = 0; c < NCH; ++c) g[c] = __any_sync(0xffffffffu, incut[c]) ? g_direct64(r[c] * a.inv2rs) : 0.0;
     } else {
-    double eu[NCH], fi[NCH];
+    double fi[NCH];
     int idx[NCH];
 #pragma unroll
     for (int c = 0; c < NCH; ++c) {
-        const double u = r[c] * a.uk;                  // node units
-        const double um = u + MAGIC64;                 // nearest node (A14)
+        const double um = fma(r[c], a.uk, MAGIC64);    // u = r uk in node units; + 1.5 * 2^52 rounds to the nearest node (A14)
         fi[c] = um - MAGIC64;
-        eu[c] = u - fi[c];                             // |eu| <= 1/2
         idx[c] = min(__double2loint(um), a.tn);        // beyond the table only for pairs the cut discards anyway
     }
     if (GMODE == G64_COEF) {
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
+            const double eu = fma(r[c], a.uk, -fi[c]);     // |eu| <= 1/2, one rounding
             const double* t = tab + idx[c] * TAB_STRIDE;
             double p = t[LEVEL];
 #pragma unroll
-            for (int k = LEVEL - 1; k >= 0; --k) p = fma(p, eu[c], t[k]);
+            for (int k = LEVEL - 1; k >= 0; --k) p = fma(p, eu, t[k]);
             g[c] = p;
         }
     } else {
@@ -92,7 +95,8 @@ __device__ __forceinline__ void g_eval(const P64Args& a, const double* __restric
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
             const double2 te = reinterpret_cast<const double2*>(tab)[idx[c]];
-            const double xi = fi[c] * a.h, e = eu[c] * a.h;
+            const double xi = fi[c] * a.h;                 // the node
+            const double e = fma(r[c], a.inv2rs, -xi);     // eps = x - x_i, one rounding
             const double xi2 = xi * xi;
             double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1), Horner from the highest kept level
             if (LEVEL >= 4) poly = -xi * fma(fma(xi2, 1.0 / 3.0, -1.5), xi2, 1.0);
@@ -186,6 +190,7 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
         constexpr int NCH = U * T;
         auto step = [&](const int j, const bool image) {
             double dx[NCH], dy[NCH], dz[NCH], r2[NCH], r[NCH], idr[NCH], gm[NCH], g[NCH];
+            bool incut[NCH];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const double4 s = src[j + u * HS];
@@ -206,12 +211,15 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
                 r2[c] = fma(dx[c], dx[c], fma(dy[c], dy[c], fma(dz[c], dz[c], a.r2add)));
                 idr[c] = rsqrt64(r2[c]);
                 r[c] = r2[c] * idr[c];
+                // the cut (A8): positive doubles order like their bit patterns, so the compare runs on the integer
+                // pipe instead of taking a slot of the FP64 pipe
+                incut[c] = __double_as_longlong(r2[c]) < __double_as_longlong(a.rcut2);
             }
-            g_eval<GMODE, LEVEL, NCH>(a, tab, r, g);
+            g_eval<GMODE, LEVEL, NCH>(a, tab, r, incut, g);
 #pragma unroll
             for (int c = 0; c < NCH; ++c) {
                 const double v = (gm[c] * idr[c]) * (idr[c] * idr[c]) * g[c];
-                const double w = r2[c] < a.rcut2 ? v : 0.0;      // the cut (A8); also drops what g did beyond its range
+                const double w = incut[c] ? v : 0.0;             // also drops what g did beyond its range
                 const int t = c % T;
                 px[t] = fma(w, dx[c], px[t]); py[t] = fma(w, dy[c], py[t]); pz[t] = fma(w, dz[c], pz[t]);
             }

@@ -65,11 +65,18 @@ def test_replicas_have_their_own_seed():
 
 def test_flop_convention_matches_design():
     import bench
-    assert bench.flops_per_pair("poly", 12) == 46.0      # (8+12) FFMA x 2 + 3 FADD + 2 FMUL + 1 MUFU
-    assert bench.flops_per_pair("poly", 13) == 48.0
+    assert bench.flops_per_pair("fp32", "poly", poly_degree=12) == 46.0   # (8+12) FFMA x 2 + 3 FADD + 2 FMUL + 1 MUFU
+    assert bench.flops_per_pair("mixed", "poly", poly_degree=13) == 48.0
+    assert bench.flops_per_pair("fp32", "table") == 35.0                  # 512 nodes / T[2]
+    assert bench.flops_per_pair("fp64", "table", table_level=4, table_layout="coef") == 42.0
+    assert bench.flops_per_pair("fp64", "table", table_level=4) == 57.0
     assert bench.PAPER_FLOPS_PER_PAIR == 51.0
     # peak = SMs x lanes x 2 x clock
-    assert bench.SM_COUNT * bench.FP32_LANES_PER_SM * 2 * 1.965e9 == pytest.approx(74.45e12, rel=1e-4)
+    assert bench.peak_tflops("fp32", 1965.0) == pytest.approx(74.45, rel=1e-4)
+    assert bench.peak_tflops("fp64", 1965.0) == pytest.approx(37.2, rel=1e-3)
+    # roofline.traffic comes from a committed ncu summary or is null, never a constant in bench.py
+    t, src = bench.ncu_traffic("no_such_workload", 32, "fp32", "poly")
+    assert t is None and src is None
 
 
 def test_headline_params_follow_the_config():
@@ -77,7 +84,7 @@ def test_headline_params_follow_the_config():
     from paper_2107_14008_b200 import workloads
     p = bench.headline_params(workloads.CONFIGS[4])
     assert (p["n_pm"], p["maxleaf"], p["precision"], p["g_mode"]) == (256, 32, "fp32", "poly")
-    assert p["close_pair_radius"] == 0.0
+    assert p["close_pair_radius"] == pytest.approx(5e-4 * 6 * 1.2 / 256)
     p1 = bench.headline_params(workloads.CONFIGS[1])
     assert p1["close_pair_radius"] == pytest.approx(0.02 * 6 * 1.2 / 32)
 
@@ -98,6 +105,22 @@ def test_poly_g_against_oracle_T(oracle, degree, bound):
     assert err == pytest.approx(dev, rel=0.05, abs=1e-12)     # the library's own error estimate is honest
     # Newtonian limit and the value at the cut
     assert g[0] == 1.0
+    assert g[-1] == pytest.approx(4.39849652838829e-4, abs=bound)
+
+
+@pytest.mark.parametrize("degree,bound", [(9, 6e-7), (10, 1.5e-7), (11, 4e-8)])
+def test_fused_g_against_oracle_T(oracle, degree, bound):
+    """The hand-fused direct evaluation (host-only hook of the library): g(r) = exp(-x^2) H(t), H ~ erfcx(x) + 2x/sqrt(pi),
+    t = 2x/3 - 1, against Eq. 1 as the oracle evaluates it."""
+    from paper_2107_14008_b200 import build, binding
+    build.build()
+    coeffs, err = binding.fused_fit(degree, 6.0)
+    x = np.linspace(0.0, 3.0, 6001)
+    g = np.exp(-x * x) * np.polyval(coeffs[::-1], 2.0 * x / 3.0 - 1.0)
+    dev = np.abs(g - oracle.oracle_T(x)).max()
+    assert dev <= bound
+    assert err == pytest.approx(dev, rel=0.05, abs=1e-12)
+    assert g[0] == pytest.approx(1.0, abs=bound)
     assert g[-1] == pytest.approx(4.39849652838829e-4, abs=bound)
 
 
