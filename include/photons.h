@@ -199,6 +199,25 @@ int photons_poly_fit(int degree, double rcut_over_rs, double* coeffs, double* ma
  * kernels use g(r) ~= exp(-x^2) * sum_k coeffs[k] t^k.  Arguments, output and errors as photons_poly_fit. */
 int photons_fused_fit(int degree, double rcut_over_rs, double* coeffs, double* max_err_g);
 
+/* Truncated multipole-to-local operator, fp64 (§2; A24-A26): for every target cell B and
+ * every source cell A in its list,
+ *     L_n(z_B) += sum_{|m| <= p - |n|} M_m(z_A) D_{n+m}(z_B - z_A - s L),    D_n = grad^n [ erfc(r / 2 r_s) / r ],
+ * the derivative tensors assembled from the paper's prefactors f_(k)(x) (L51) with all trace terms (A24).
+ * Multi-indices n = (n_x, n_y, n_z), |n| <= p, are ordered by |n|, then n_x descending, then n_y descending; there are
+ * NC = (p+1)(p+2)(p+3)/6 of them.  Multipoles carry the Taylor factors, M_m = sum_j m_j (-a_j)^m / m! (A25).
+ *   p            expansion order, 0..4 (the paper does not state its order; A26)
+ *   centres      n_cells x 3;  multipoles, locals: n_cells x NC, row-major doubles (locals is overwritten)
+ *   pair_ptr     n_cells + 1 offsets into pair_src (CSR by target cell);  pair_src: source cell of each pair
+ *   pair_shift   3 signed bytes per pair, s in {-1, 0, +1} box lengths added to the source centre, or NULL
+ *   mem_kind     all arrays host or all device (PHOTONS_MEM_*); host arrays are copied in and out
+ *   cuda_stream  a cudaStream_t (NULL = default stream); the call returns after the work has completed
+ *   kernel_ms    (may be NULL) CUDA-event time of the kernel
+ * A source at zero separation from its target is not allowed (the list holds well-separated cells).
+ * Errors: EINVAL, ENODEVICE, ENOMEM, ECUDA. */
+int photons_m2l(int device, int p, double r_s, double boxsize, long long n_cells, const double* centres,
+                const double* multipoles, const long long* pair_ptr, const int* pair_src, const signed char* pair_shift,
+                double* locals, int mem_kind, void* cuda_stream, double* kernel_ms);
+
 /* Message of the last failing call on ctx; valid until the next call on ctx. */
 const char* photons_last_error(const photons_ctx* ctx);
 

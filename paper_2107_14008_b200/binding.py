@@ -29,7 +29,7 @@ ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX",
 EXPORTS = [
     "photons_default_params", "photons_create", "photons_set_stream", "photons_set_particles", "photons_build_leaves",
     "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
-    "photons_peak_probe", "photons_poly_fit", "photons_fused_fit", "photons_last_error", "photons_destroy",
+    "photons_peak_probe", "photons_poly_fit", "photons_fused_fit", "photons_m2l", "photons_last_error", "photons_destroy",
 ]
 
 
@@ -100,6 +100,9 @@ def load():
     lib.photons_poly_fit.argtypes = [ci, ctypes.c_double, vp, ctypes.POINTER(ctypes.c_double)]
     lib.photons_fused_fit.restype = ci
     lib.photons_fused_fit.argtypes = [ci, ctypes.c_double, vp, ctypes.POINTER(ctypes.c_double)]
+    lib.photons_m2l.restype = ci
+    lib.photons_m2l.argtypes = [ci, ci, ctypes.c_double, ctypes.c_double, ll, vp, vp, vp, vp, vp, vp, ci, vp,
+                                ctypes.POINTER(ctypes.c_double)]
     lib.photons_last_error.restype = ctypes.c_char_p
     lib.photons_last_error.argtypes = [vp]
     lib.photons_destroy.restype = None
@@ -273,6 +276,50 @@ def fused_fit(degree: int, rcut_over_rs: float = 6.0):
     if rc != OK:
         raise PhotonsError(rc, "fused_fit: bad argument")
     return coeffs, err.value
+
+
+def m2l_n_coeffs(p: int) -> int:
+    return (p + 1) * (p + 2) * (p + 3) // 6
+
+
+def m2l(centres, multipoles, pair_ptr, pair_src, pair_shift=None, *, p, r_s, boxsize=0.0, out=None, device=0, stream=None):
+    """photons_m2l: numpy arrays (host) or torch CUDA tensors (device), all of one kind.  Returns (locals, kernel_ms)."""
+    def ptr(x, dtype_np, dtype_name):
+        if x is None:
+            return None, MEM_HOST, None
+        if _is_tensor(x):
+            if str(x.dtype) != "torch." + dtype_name or not x.is_contiguous():
+                raise TypeError(f"contiguous {dtype_name} tensor expected")
+            return x.data_ptr(), (MEM_DEVICE if x.is_cuda else MEM_HOST), x
+        a = np.ascontiguousarray(x, dtype=dtype_np)
+        return a.ctypes.data, MEM_HOST, a
+    n_cells = int(centres.shape[0])
+    nc = m2l_n_coeffs(p)
+    if tuple(multipoles.shape) != (n_cells, nc):
+        raise ValueError("multipoles must be n_cells x NC(p)")
+    c_ptr, kind, k0 = ptr(centres, np.float64, "float64")
+    m_ptr, kind_m, k1 = ptr(multipoles, np.float64, "float64")
+    pp_ptr, kind_p, k2 = ptr(pair_ptr, np.int64, "int64")
+    ps_ptr, kind_s, k3 = ptr(pair_src, np.int32, "int32")
+    sh_ptr, _, k4 = ptr(pair_shift, np.int8, "int8")
+    if len({kind, kind_m, kind_p, kind_s}) != 1:
+        raise ValueError("all arrays must be of one memory kind")
+    if out is None:
+        if kind == MEM_DEVICE:
+            import torch
+            out = torch.empty((n_cells, nc), dtype=torch.float64, device=centres.device)
+        else:
+            out = np.empty((n_cells, nc), dtype=np.float64)
+    o_ptr, kind_o, k5 = ptr(out, np.float64, "float64")
+    if kind_o != kind:
+        raise ValueError("out must be of the inputs' memory kind")
+    ms = ctypes.c_double()
+    handle = getattr(stream, "cuda_stream", stream)
+    rc = load().photons_m2l(device, int(p), float(r_s), float(boxsize), n_cells, c_ptr, m_ptr, pp_ptr, ps_ptr, sh_ptr, o_ptr,
+                            kind, ctypes.c_void_p(handle or 0), ctypes.byref(ms))
+    if rc != OK:
+        raise PhotonsError(rc, "photons_m2l failed")
+    return out, ms.value
 
 
 def short_range_acc(pos, mass=None, *, out=None, **params):

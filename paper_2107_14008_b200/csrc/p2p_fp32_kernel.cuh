@@ -241,8 +241,8 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
 }
 
 // Exact path (A12): one target against one staged run of sources, in fp64 from the exact coordinates with
-// the library's erfc / exp — the oracle's arithmetic.  Sources j = first, first + step, ... < ns of the run at e.x.
-// Returns the acceleration in caller units.
+// the library's erfc / exp — the oracle's arithmetic.  The lane's share of the run at e.x, exactly as the fast path
+// deals it out: source PAIRS first, first + step, ... (sources 2p and 2p + 1).  Returns the acceleration in caller units.
 static __device__ __noinline__ double3 exact_run(const P32Args& a, int tslot, uint2 e, int first, int step)
 {
     const int ns = (int)(e.y & 0xffffu);
@@ -250,7 +250,8 @@ static __device__ __noinline__ double3 exact_run(const P32Args& a, int tslot, ui
     const double sx = a.Ld * ((int)((e.y >> 16) & 3u) - 1), sy = a.Ld * ((int)((e.y >> 18) & 3u) - 1), sz = a.Ld * ((int)((e.y >> 20) & 3u) - 1);
     const double4 pi = a.p64[tslot];
     double ax = 0, ay = 0, az = 0;
-    for (int j = first; j < ns; j += step) {
+    for (int jj = 2 * first; jj < ns; jj += 2 * step)
+    for (int j = jj; j < jj + 2; ++j) {
         const double4 pj = a.p64[e.x + j];
         double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (per_pair) {

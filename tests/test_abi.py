@@ -22,7 +22,7 @@ def _header():
 
 
 def _declared():
-    return sorted(set(re.findall(r"\b(photons_[a-z_]+)\s*\(", _header())))
+    return sorted(set(re.findall(r"\b(photons_[a-z0-9_]+)\s*\(", _header())))
 
 
 def test_header_symbols_are_exported(lib):
@@ -79,6 +79,32 @@ def test_no_cpu_fallback_without_a_device(lib):
     assert e.value.code == B.ENODEVICE
     out = ctypes.c_double()
     assert lib.photons_peak_probe(0, 0, ctypes.byref(out)) != B.OK
+
+
+def test_generated_m2l_header_is_in_sync_with_its_generator():
+    import importlib.util
+    path = os.path.join(ROOT, "paper_2107_14008_b200", "csrc", "gen_m2l.py")
+    spec = importlib.util.spec_from_file_location("gen_m2l", path)
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    assert open(os.path.join(os.path.dirname(path), "m2l_generated.cuh")).read() == gen.render()
+
+
+def test_m2l_argument_checks_need_no_device(lib):
+    import numpy as np
+    from paper_2107_14008_b200 import binding as B
+    c = np.zeros((2, 3)); c[1, 0] = 1.0
+    ptr = np.array([0, 1, 1], dtype=np.int64)
+    src = np.array([1], dtype=np.int32)
+    with pytest.raises(B.PhotonsError) as e:
+        B.m2l(c, np.zeros((2, B.m2l_n_coeffs(5))), ptr, src, p=5, r_s=0.1)        # order above 4
+    assert e.value.code == B.EINVAL
+    with pytest.raises(B.PhotonsError) as e:
+        B.m2l(c, np.zeros((2, 4)), ptr, src, p=1, r_s=-1.0)
+    assert e.value.code == B.EINVAL
+    with pytest.raises(ValueError):
+        B.m2l(c, np.zeros((2, 5)), ptr, src, p=1, r_s=0.1)
+    assert [B.m2l_n_coeffs(p) for p in range(5)] == [1, 4, 10, 20, 35]
 
 
 def test_product_does_not_touch_the_oracle():
