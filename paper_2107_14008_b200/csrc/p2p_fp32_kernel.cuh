@@ -243,27 +243,29 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
 // Exact path (A12): one target against one staged run of sources, in fp64 from the exact coordinates with
 // the library's erfc / exp — the oracle's arithmetic.  The lane's share of the run at e.x, exactly as the fast path
 // deals it out: source PAIRS first, first + step, ... (sources 2p and 2p + 1).  Returns the acceleration in caller units.
-static __device__ __noinline__ double3 exact_run(const P32Args& a, int tslot, uint2 e, int first, int step)
+// (scalars by value: a reference to the kernel's parameter block would make the compiler copy it to local memory)
+static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64, double Ld, double eps2_d, double rcut2_d,
+                                                 double inv2rs_d, int tslot, uint2 e, int first, int step)
 {
     const int ns = (int)(e.y & 0xffffu);
     const bool per_pair = (e.y & ENTRY_PER_PAIR) != 0;
-    const double sx = a.Ld * ((int)((e.y >> 16) & 3u) - 1), sy = a.Ld * ((int)((e.y >> 18) & 3u) - 1), sz = a.Ld * ((int)((e.y >> 20) & 3u) - 1);
-    const double4 pi = a.p64[tslot];
+    const double sx = Ld * ((int)((e.y >> 16) & 3u) - 1), sy = Ld * ((int)((e.y >> 18) & 3u) - 1), sz = Ld * ((int)((e.y >> 20) & 3u) - 1);
+    const double4 pi = p64[tslot];
     double ax = 0, ay = 0, az = 0;
     for (int jj = 2 * first; jj < ns; jj += 2 * step)
     for (int j = jj; j < jj + 2; ++j) {
-        const double4 pj = a.p64[e.x + j];
+        const double4 pj = p64[e.x + j];
         double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (per_pair) {
-            dx -= a.Ld * rint(dx / a.Ld); dy -= a.Ld * rint(dy / a.Ld); dz -= a.Ld * rint(dz / a.Ld);
+            dx -= Ld * rint(dx / Ld); dy -= Ld * rint(dy / Ld); dz -= Ld * rint(dz / Ld);
         } else {
             dx += sx; dy += sy; dz += sz;
         }
         const double r2 = dx * dx + dy * dy + dz * dz;
-        const double r2e = r2 + a.eps2_d;
-        if (r2 > 0.0 && r2e < a.rcut2_d) {
+        const double r2e = r2 + eps2_d;
+        if (r2 > 0.0 && r2e < rcut2_d) {
             const double r = sqrt(r2e);
-            const double x = r * a.inv2rs_d;
+            const double x = r * inv2rs_d;
             const double w = pj.w * (erfc(x) + 1.1283791670955125739 * x * exp(-x * x)) / (r2e * r);
             ax += w * dx; ay += w * dy; az += w * dz;
         }
@@ -274,7 +276,7 @@ static __device__ __noinline__ double3 exact_run(const P32Args& a, int tslot, ui
 // ---------------------------------------------------------------------------------------------------------
 
 template <int T, int HS, bool MIXED, int GKIND, int GPAR>
-__global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
+__global__ void __launch_bounds__(256, T == 1 ? 3 : 1) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
@@ -497,7 +499,7 @@ __global__ void __launch_bounds__(256) p2p_fp32_kernel(P32Args a)
 #pragma unroll
             for (int t = 0; t < T; ++t) {
                 if (fmaf(px[t], px[t], fmaf(py[t], py[t], pz[t] * pz[t])) > a.pth2) {
-                    const double3 x = exact_run(a, tslot[t], e, half, pstep);
+                    const double3 x = exact_run(a.p64, a.Ld, a.eps2_d, a.rcut2_d, a.inv2rs_d, tslot[t], e, half, pstep);
                     ax[t] += x.x * a.inv_oscale; ay[t] += x.y * a.inv_oscale; az[t] += x.z * a.inv_oscale;
                     px[t] = py[t] = pz[t] = 0.f;
                 }
