@@ -58,8 +58,8 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
             return 2.0 * 74 + 17 + 12 + 3
         if table_layout == "coef":  # level 4: 15 DFMA + 7 DMUL + 4 DADD + 1 MUFU; one DFMA per level
             return 2.0 * (11 + table_level) + 7 + 4 + 1
-        # paper layout: level 4: 20 DFMA + 12 DMUL + 4 DADD + 1 MUFU; level 3: 18 + 11 + 4 + 1
-        return {4: 57.0, 3: 52.0}.get(table_level, 52.0 - 4.0 * (3 - table_level))
+        # paper layout: level 4: 20 DFMA + 11 DMUL + 4 DADD + 1 MUFU; level 3: 18 + 10 + 4 + 1
+        return {4: 56.0, 3: 51.0}.get(table_level, 51.0 - 4.0 * (3 - table_level))
     if g_mode == "poly":           # (8 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
         return 2.0 * (8 + poly_degree) + 3 + 2 + 1
     if g_mode == "table":          # 512 nodes, level 2: 9 FFMA + 6 FADD + 10 FMUL + 1 MUFU
@@ -501,6 +501,63 @@ def run_streams_study(args):
     return 0
 
 
+def run_m2l(args):
+    """Truncated M2L: cell pairs per second of photons_m2l at order p on a periodic lattice
+    of n^3 cells (jittered centres, cell = 1 PM cell so r_s = 1.2 cells), every target taking the 316 sources at Chebyshev
+    distance 2..3 - the shape of an FMM interaction list ("children of the parent's neighbours"); random multipoles.
+    Parity of the same call is in tests/test_gpu_m2l.py; the oracle leg times oracle/m2l.py on a bounded sample."""
+    import torch
+    from paper_2107_14008_b200 import binding as B
+    n, p = args.m2l_cells, args.m2l_order
+    rng = np.random.default_rng(77)
+    g = np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), axis=-1).reshape(-1, 3)
+    centres = (g + 0.5 + 0.2 * (rng.random((n ** 3, 3)) - 0.5)) / n
+    off = np.array([(i, j, k) for i in range(-3, 4) for j in range(-3, 4) for k in range(-3, 4) if max(abs(i), abs(j), abs(k)) >= 2])
+    nb = g[:, None, :] + off[None, :, :]
+    shift = np.floor_divide(nb, n).astype(np.int8)            # source moved by this many box lengths
+    nbw = np.mod(nb, n)
+    src = (nbw[..., 0] * n * n + nbw[..., 1] * n + nbw[..., 2]).astype(np.int32).reshape(-1)
+    ptr = np.arange(0, (n ** 3 + 1) * len(off), len(off), dtype=np.int64)
+    nc = B.m2l_n_coeffs(p)
+    M = rng.normal(size=(n ** 3, nc)) * (0.4 / n) ** np.array([sum(q) for q in _m2l_indices(p)])
+    r_s = 1.2 / n
+    d = [torch.from_numpy(x).cuda() for x in (centres, M, ptr, src, np.ascontiguousarray(shift.reshape(-1, 3)))]
+    out = torch.empty((n ** 3, nc), dtype=torch.float64, device="cuda")
+    ms = []
+    for it in range(args.warmup + args.steps):
+        _, t = B.m2l(d[0], d[1], d[2], d[3], d[4], p=p, r_s=r_s, boxsize=1.0, out=out)
+        if it >= args.warmup:
+            ms.append(t)
+    n_pairs = len(src)
+    k_ms = float(np.median(ms))
+    flops = {4: 749.0}.get(p)          # SASS count of m2l_kernel<4> (profiles/r2_sass_inner_loop.md)
+    line = {"metric": "truncated M2L cell pairs/s", "value": n_pairs / (k_ms * 1e-3), "unit": "cell pairs/s", "order_p": p, "n_cells": n ** 3,
+            "n_pairs": n_pairs, "kernel_ms": k_ms, "dtype": "f64",
+            "roofline": None if flops is None else {"bound": "alu", "achieved": n_pairs * flops / (k_ms * 1e-3) / 1e12, "peak": peak_tflops("fp64", 1965.0),
+                                                    "unit": "TFLOP/s", "frac": n_pairs * flops / (k_ms * 1e-3) / 1e12 / peak_tflops("fp64", 1965.0),
+                                                    "flops_per_pair": flops}}
+    if not args.no_cpu_baseline:
+        import oracle
+        import time
+        tsel = rng.choice(n ** 3, size=min(n ** 3, 2000), replace=False)
+        pairs = np.stack([np.repeat(tsel, len(off)), src.reshape(-1, len(off))[tsel].reshape(-1)], axis=1)
+        sh = shift.reshape(-1, len(off), 3)[tsel].reshape(-1, 3)
+        t0 = time.perf_counter()
+        ref = oracle.m2l.m2l(centres, M, pairs, p, r_s, boxsize=1.0, shifts=sh)
+        dt = time.perf_counter() - t0
+        got = out.cpu().numpy()
+        err = float((np.abs(got[tsel] - ref[tsel]).max(axis=0) / np.abs(ref[tsel]).max(axis=0)).max())
+        line["cpu_baseline"] = {"value": len(pairs) / dt, "unit": "cell pairs/s", "cores": 1, "kind": "oracle",
+                                "sample": f"{len(tsel)} target cells x {len(off)} sources (numpy fp64)"}
+        line["max_rel_err_vs_oracle"] = err
+    print(json.dumps(line))
+    return 0
+
+
+def _m2l_indices(p):
+    return [(nx, ny, k - nx - ny) for k in range(p + 1) for nx in range(k, -1, -1) for ny in range(k - nx, -1, -1)]
+
+
 def run_table_study(args):
     """Eq. 2 study (Fig. 2): every table size x Taylor level, fp32 and fp64, on one workload:
     force error against the oracle and kernel time.  Prints a markdown table (see profiles/)."""
@@ -562,6 +619,9 @@ def main(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (ncu captures)")
     ap.add_argument("--streams-study", action="store_true", help="kernel and step time for 1/2/4 streams (a10)")
+    ap.add_argument("--m2l", action="store_true", help="truncated M2L kernel (SURVEY §8(f) 4) instead of the P2P bench line")
+    ap.add_argument("--m2l-cells", type=int, default=48, help="cells per side of the M2L lattice")
+    ap.add_argument("--m2l-order", type=int, default=4)
     ap.add_argument("--sweep", action="store_true", help="MAXLEAF x g-mode x precision table instead of the bench line")
     ap.add_argument("--table-study", action="store_true", help="Eq. 2: table size x Taylor level, fp32 and fp64")
     ap.add_argument("--sweep-targets", type=int, default=1000)
@@ -571,6 +631,8 @@ def main(argv=None):
         ap.error("--steps >= 1 and --warmup >= 0")
     if args.precision == "fp64" and args.g_mode in ("poly", "fused"):
         args.g_mode = "direct"           # POLY and FUSED are fp32 approximations
+    if args.m2l:
+        return run_m2l(args)
     if args.streams_study:
         return run_streams_study(args)
     if args.sweep:

@@ -111,9 +111,10 @@ typedef struct {
                                  taken at r_eps = sqrt(r^2 + eps^2), a_i += G m_j d_ij g(r_eps) / r_eps^3 for pairs with
                                  0 < r and r_eps < r_cut.  0 = none (default; north_star's formula) */
     int table_layout;         /* TABLE: PHOTONS_TABLE_PAPER (default) or PHOTONS_TABLE_COEF */
-    int leaf_order;           /* order in which CTAs take the target leaves: 0 = longest source list first (default; shortens
-                                 the tail of clustered loads), 1 = ORB order (neighbouring leaves run together: their
-                                 source leaves are shared in L2) */
+    int leaf_order;           /* order in which CTAs take the target leaves: 0 = ORB order (default: neighbouring leaves run
+                                 together and share their source leaves in L2), 1 = longest source list first */
+    int orb_method;           /* upper levels of the ORB build: 0 = radix-select partition of every node about its median
+                                 (default), 1 = one full radix sort of (node, coordinate) keys per level (round-1 path) */
 } photons_params;
 
 typedef struct {
@@ -123,7 +124,8 @@ typedef struct {
     long long n_leaf_pairs;    /* (target leaf, source leaf) tasks, the paper's Task list length (L77) */
     long long pairs_evaluated; /* sum over tasks of n_i * n_j, real particles only (paper's count, L218; A18) */
     long long max_leaves_per_target; /* longest source list, in leaves */
-    double build_ms;           /* last photons_build_leaves, host wall clock incl. device sync */
+    double build_ms;           /* last photons_build_leaves: CUDA-event time of its device work (the call itself returns
+                                  once that work is enqueued; the value is read at the next synchronisation) */
     double kernel_ms;          /* last photons_short_range_acc: CUDA-event time of the P2P launches alone */
     double total_ms;           /* last photons_short_range_acc: host wall clock incl. copies and sync */
     long long kernel_launches; /* kernels of this library launched on ctx since photons_create (the CUB sort and

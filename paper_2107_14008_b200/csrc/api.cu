@@ -92,6 +92,16 @@ __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Ti
     if ((threadIdx.x & 31) == 0 && mb > 0) atomicMax(&flags[1], mb);
 }
 
+// build_ms from the events recorded around photons_build_leaves' device work
+static void resolve_build_ms(Ctx* c)
+{
+    if (!c->build_ms_pending) return;
+    float ms = 0;
+    if (cudaEventSynchronize(c->evb1) == cudaSuccess && cudaEventElapsedTime(&ms, c->evb0, c->evb1) == cudaSuccess) c->stats.build_ms = ms;
+    else cudaGetLastError();
+    c->build_ms_pending = false;
+}
+
 static void free_particles(Ctx* c)
 {
     c->d_pos = nullptr;     // the buffers stay in the workspace
@@ -130,6 +140,7 @@ void photons_default_params(photons_params* p)
     p->softening = 0.0;
     p->table_layout = PHOTONS_TABLE_PAPER;
     p->leaf_order = 0;
+    p->orb_method = 0;
 }
 
 static int create_fail(char* err_buf, int err_len, int code, const char* msg)
@@ -164,6 +175,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         if (p.table_layout == PHOTONS_TABLE_COEF && p.precision != PHOTONS_FP64)
             return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF is an option of the PHOTONS_FP64 path");
     }
+    if (p.orb_method != 0 && p.orb_method != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "orb_method must be 0 or 1");
     if (p.leaf_order != 0 && p.leaf_order != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "leaf_order must be 0 or 1");
     if (p.n_streams < 1 || p.n_streams > 64) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "n_streams must be 1..64");
     if (p.close_pair_radius < 0 || !std::isfinite(p.close_pair_radius)) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be >= 0");
@@ -226,6 +238,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
     }
     c->own_stream0 = c->streams[0];
     ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+    ok = ok && cudaEventCreate(&c->evb0) == cudaSuccess && cudaEventCreate(&c->evb1) == cudaSuccess;
     int rc = PHOTONS_OK;
     if (!ok) rc = fail(c, PHOTONS_ECUDA, "stream/event creation failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == PHOTONS_OK && p.g_mode == PHOTONS_G_TABLE) rc = make_table(c);
@@ -308,11 +321,12 @@ int photons_build_leaves(photons_ctx* ctx)
     if (!c) return PHOTONS_EINVAL;
     if (c->n < 1) return fail(c, PHOTONS_ESTATE, "build_leaves: call set_particles first");
     PH_CUDA(c, cudaSetDevice(c->p.device));
-    const double t0 = now_ms();
     free_leaves(c);
+    PH_CUDA(c, cudaEventRecord(c->evb0, c->streams[0]));
     int rc = build_leaves_impl(c);
     if (rc != PHOTONS_OK) { free_leaves(c); return rc; }
-    c->stats.build_ms = now_ms() - t0;
+    PH_CUDA(c, cudaEventRecord(c->evb1, c->streams[0]));
+    c->build_ms_pending = true;      // the tail of the build is still in flight: no host synchronisation here
     c->leaves_built = true;
     return PHOTONS_OK;
 }
@@ -384,6 +398,7 @@ int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind
     float ms = 0;
     cudaEventElapsedTime(&ms, c->ev0, c->ev1);
     c->stats.kernel_ms = ms;
+    resolve_build_ms(c);
     c->stats.total_ms = now_ms() - t0;
     c->stats.kernel_launches = c->launches;
     if (stats) *stats = c->stats;
@@ -427,6 +442,7 @@ int photons_get_stats(photons_ctx* ctx, photons_stats* stats)
 {
     Ctx* c = reinterpret_cast<Ctx*>(ctx);
     if (!c || !stats) return PHOTONS_EINVAL;
+    resolve_build_ms(c);
     c->stats.kernel_launches = c->launches;
     *stats = c->stats;
     return PHOTONS_OK;
@@ -454,6 +470,8 @@ void photons_destroy(photons_ctx* ctx)
     for (auto e : c->stream_done) if (e) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->evb0) cudaEventDestroy(c->evb0);
+    if (c->evb1) cudaEventDestroy(c->evb1);
     delete c;
 }
 

@@ -49,6 +49,7 @@ enum WsSlot {
     WS_POS, WS_MASS, WS_IN_POS, WS_IN_MASS, WS_FLAG, WS_OUT,
     WS_PERM, WS_ORB_P0, WS_ORB_P1, WS_ORB_KEYS, WS_ORB_KEYS2, WS_ORB_VALS, WS_ORB_VALS2, WS_ORB_LO, WS_ORB_HI, WS_CUB_TMP,
     WS_LEAF_CNT, WS_NODE_LO, WS_NODE_HI, WS_NODE_BOX32, WS_LEAF_CTR, WS_SLOT_SRC, WS_P64, WS_P32,
+    WS_SEL_NODE, WS_SEL_CNT, WS_SEL_Q0, WS_SEL_C0, WS_SEL_HIST, WS_SEL_NODEVAR, WS_SEL_CNT2, WS_SEL_BASE2, WS_SEL_LO2, WS_SEL_HI2,
     WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_LIST_STASH, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
     WS_COUNT
 };
@@ -68,6 +69,8 @@ struct Ctx {
     cudaStream_t own_stream0 = nullptr;  // the stream created for slot 0 (destroyed with the context)
     long long launches = 0;              // kernels of this library launched so far (cub's are not counted)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t evb0 = nullptr, evb1 = nullptr;   // around the device work of build_leaves
+    bool build_ms_pending = false;
     std::vector<cudaEvent_t> stream_done;
 
     // particles in caller order (wrapped into [0, L))
@@ -101,6 +104,10 @@ struct Ctx {
     double fused_err = 0;               // max |exp(-x^2) H_poly(x) - g| over [0, x_cut] in exact arithmetic
 
     DevBuf ws[WS_COUNT];
+    // chunk tables of the ORB partition levels (orb_select.cu): they depend on (n, L0) only
+    long long sel_n = -1;
+    int sel_L0 = -1;
+    std::vector<long long> sel_off, sel_noff;
 
     photons_stats stats{};
     std::string err;
@@ -122,6 +129,8 @@ cudaError_t opt_in_smem(Ctx* c, const void* kernel, size_t bytes);
                                  "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
     } while (0)
 
+// orb_select.cu
+int orb_phase_a_select(Ctx* c, int L0, float4*& P_cur, float4*& P_alt, int* lo, int* hi, cudaStream_t st);
 // build.cu
 int build_leaves_impl(Ctx* c);
 void free_leaves(Ctx* c);

@@ -25,6 +25,9 @@ namespace photons {
 
 constexpr double R2_FLOOR64 = 0x1p-600;   // start of every r^2 chain: 1/r^3 = 2^900 stays finite, w * 0 = 0 (A7)
 constexpr double MAGIC64 = 6755399441055744.0;   // 1.5 * 2^52
+// ring depth of the fp64 kernels: a stage is 4 KB per warp, and with 2 stages a fourth CTA fits per SM (measured:
+// table 512/T[4] 262.8 -> 252.8 ms on config 4)
+constexpr int N_STAGES64 = 2;
 constexpr int TAB_STRIDE = 5;             // doubles per node in the coefficient layout (odd: fewer bank conflicts)
 
 enum { G64_DIRECT = 0, G64_TABLE = 1, G64_COEF = 2 };
@@ -41,6 +44,7 @@ struct P64Args {
     const double* table;      // TABLE: {T_i, E_i} pairs; COEF: TAB_STRIDE doubles per node; i = 0..tn
     int tn, tab_doubles;      // number of doubles to stage in shared memory
     double uk, h;             // u = r * uk in node units; h = 3 / tn
+    float hf;                 // (float) h
     void* out;                // caller order, n x 3
     int out_f32;
 };
@@ -98,11 +102,19 @@ __device__ __forceinline__ void g_eval(const P64Args& a, const double* __restric
             const double xi = fi[c] * a.h;                 // the node
             const double e = fma(r[c], a.inv2rs, -xi);     // eps = x - x_i, one rounding
             const double xi2 = xi * xi;
-            double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1), Horner from the highest kept level
-            if (LEVEL >= 4) poly = -xi * fma(fma(xi2, 1.0 / 3.0, -1.5), xi2, 1.0);
-            if (LEVEL >= 3) poly = fma(poly, e, fma(fma(xi2, 2.0 / 3.0, -5.0 / 3.0), xi2, 1.0 / 3.0));
-            if (LEVEL >= 2) poly = fma(poly, e, fma(-xi, xi2, xi));
-            if (LEVEL >= 1) poly = fma(poly, e, xi2);
+            double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1)
+            if (LEVEL >= 3) {
+                // T[3] + T[4] are below (h/2)^2 = 1e-5 of T[1] + T[2]: their bracket e^2 (c_3 + e c_4) is evaluated in
+                // fp32 on the FMA pipe (relative error 1e-7 of a 1e-5 correction) and added once in fp64, which
+                // takes 5 instructions per pair off the FP64 pipe; T[1], T[2] and the sum stay in fp64.
+                const float xf = __int_as_float(0x4b000000 | idx[c]) - 8388608.0f;     // float(idx) without I2F
+                const float xif = xf * a.hf, xf2 = xif * xif, ef = (float)e;
+                float hi = fmaf(fmaf(xf2, 2.0f / 3.0f, -5.0f / 3.0f), xf2, 1.0f / 3.0f);
+                if (LEVEL >= 4) hi = fmaf(-xif * fmaf(fmaf(xf2, 1.0f / 3.0f, -1.5f), xf2, 1.0f), ef, hi);
+                poly = (double)(hi * ef * ef);
+            }
+            if (LEVEL >= 2) poly += fma(fma(-xi, xi2, xi), e, xi2);
+            else if (LEVEL >= 1) poly = xi2;
             g[c] = LEVEL >= 1 ? fma(te.y * e, poly, te.x) : te.x;
         }
     }
@@ -117,11 +129,11 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
     const int M = a.maxleaf;
     const int stage_bytes = a.chunk_max * 32;
-    unsigned char* ring = smem_raw + (size_t)warp * N_STAGES * stage_bytes;
-    unsigned char* tail = smem_raw + (size_t)W * N_STAGES * stage_bytes;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES;
-    uint2* meta = reinterpret_cast<uint2*>(tail + W * N_STAGES * 8) + warp * N_STAGES;
-    double* red = reinterpret_cast<double*>(tail + W * N_STAGES * 16);   // W x T x 32 x 3 doubles
+    unsigned char* ring = smem_raw + (size_t)warp * N_STAGES64 * stage_bytes;
+    unsigned char* tail = smem_raw + (size_t)W * N_STAGES64 * stage_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(tail) + warp * N_STAGES64;
+    uint2* meta = reinterpret_cast<uint2*>(tail + W * N_STAGES64 * 8) + warp * N_STAGES64;
+    double* red = reinterpret_cast<double*>(tail + W * N_STAGES64 * 16);   // W x T x 32 x 3 doubles
     double* tab = red + (size_t)W * T * 32 * 3;
 
     constexpr int HS = 32 / LG;
@@ -150,24 +162,24 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
     const int n_my = n_all > warp ? (int)((n_all - warp + W - 1) / W) : 0;
 
     if (lane == 0) {
-        for (int s = 0; s < N_STAGES; ++s) mbar_init(&bars[s], 1);
+        for (int s = 0; s < N_STAGES64; ++s) mbar_init(&bars[s], 1);
         mbar_fence_init();
     }
     __syncwarp();
     auto issue = [&](int k) {
         const uint2 e = a.chunks[c0 + warp + (long long)k * W];
-        const int st = k % N_STAGES;
+        const int st = k % N_STAGES64;
         meta[st] = e;
         const uint32_t bytes = (e.y & 0xffffu) * 32u;
         mbar_expect_tx(&bars[st], bytes);
         bulk_g2s(ring + (size_t)st * stage_bytes, a.p64 + e.x, bytes, &bars[st]);
     };
     if (lane == 0)
-        for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k);
+        for (int k = 0; k < N_STAGES64 && k < n_my; ++k) issue(k);
 
     for (int k = 0; k < n_my; ++k) {
-        const int st = k % N_STAGES;
-        mbar_wait(&bars[st], (uint32_t)(k / N_STAGES) & 1u);
+        const int st = k % N_STAGES64;
+        mbar_wait(&bars[st], (uint32_t)(k / N_STAGES64) & 1u);
         const uint2 e = meta[st];
         const int ns = (int)(e.y & 0xffffu);
         const double4* src = reinterpret_cast<const double4*>(ring + (size_t)st * stage_bytes);
@@ -232,7 +244,7 @@ __global__ void __launch_bounds__(256) p2p_fp64_kernel(P64Args a)
 #pragma unroll
         for (int t = 0; t < T; ++t) { ax[t] += px[t]; ay[t] += py[t]; az[t] += pz[t]; }
         __syncwarp();
-        if (lane == 0 && k + N_STAGES < n_my) issue(k + N_STAGES);
+        if (lane == 0 && k + N_STAGES64 < n_my) issue(k + N_STAGES64);
     }
 
 #pragma unroll
@@ -324,13 +336,14 @@ int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool ou
         a.table = coef ? c->table.d_C64 : reinterpret_cast<const double*>(c->table.d_TE64);
         a.tab_doubles = (a.tn + 1) * (coef ? TAB_STRIDE : 2);
         a.h = 3.0 / a.tn;
+        a.hf = (float)a.h;
         a.uk = a.tn / 3.0 * a.inv2rs;
     }
     a.out = out; a.out_f32 = out_f32 ? 1 : 0;
     const int W = c->p.warps_per_leaf;
     const int M = c->p.maxleaf;
     const int T = (M + 31) / 32;
-    const size_t smem = (size_t)W * N_STAGES * c->p.chunk_max * 32 + (size_t)W * N_STAGES * 16 + (size_t)W * T * 32 * 3 * 8 +
+    const size_t smem = (size_t)W * N_STAGES64 * c->p.chunk_max * 32 + (size_t)W * N_STAGES64 * 16 + (size_t)W * T * 32 * 3 * 8 +
                         (size_t)a.tab_doubles * 8;
     switch (M) {
         case 16: return launch_g<1, 16>(c, a, count, W, smem, st);
