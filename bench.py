@@ -54,8 +54,8 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
     ncu's op_ffma counters read 0 for the packed FFMA2 stream): FFMA/DFMA = 2, FADD/FMUL/DADD/DMUL = 1, MUFU = 1,
     compares and selects 0."""
     if precision == "fp64":
-        if g_mode == "direct":     # 74 DFMA + 17 DMUL + 12 DADD + 3 MUFU (library erfc + exp inlined, branch-free)
-            return 2.0 * 74 + 17 + 12 + 3
+        if g_mode == "direct":     # executed per pair on config 4 (ncu DFMA/DMUL/DADD counters): 52.6 + 12.7 + 7.8 + 3 MUFU;
+            return 129.0           # the static count is 180, warp votes skip erfc/exp where no lane is inside the cut
         if table_layout == "coef":  # level 4: 15 DFMA + 7 DMUL + 4 DADD + 1 MUFU; one DFMA per level
             return 2.0 * (11 + table_level) + 7 + 4 + 1
         # paper layout: level 4: 20 DFMA + 11 DMUL + 4 DADD + 1 MUFU; level 3: 18 + 10 + 4 + 1
@@ -66,8 +66,8 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
         return 2.0 * 9 + 6 + 10 + 1 + 2.0 * (table_level - 2)
     if g_mode == "fused":          # hand-fused erfc/exp: see profiles/r2_sass_inner_loop.md
         return FUSED_FLOPS_PER_PAIR
-    # direct = stock erfcf + expf: 31 FFMA + 16 FMUL + 8.5 FADD + 5 MUFU (3 FFMA2 + 1.5 FADD2 packed among them)
-    return 2.0 * 31 + 16 + 8.5 + 5
+    # direct = stock erfcf + expf: 31 FFMA + 16 FMUL + 10 FADD + 5 MUFU (3 FFMA2 + 1.5 FADD2 packed among them)
+    return 2.0 * 31 + 16 + 10 + 5
 
 
 FUSED_FLOPS_PER_PAIR = 2.0 * (7 + 10) + 8 + 3 + 2   # degree 10: 17 FFMA + 8 FMUL + 3 FADD + MUFU.RSQ + MUFU.EX2
@@ -80,15 +80,16 @@ def peak_tflops(precision: str, sm_mhz: float) -> float:
 
 def ncu_traffic(workload: str, maxleaf: int, precision: str, g_mode: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed `ncu --set
-    full` summaries (profiles/r2_traffic.json, each entry naming its capture and commit); null when this variant has
+    full` summaries (profiles/r2_traffic.csv, each row naming its capture and commit); null when this variant has
     none.  Never a number typed in here."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as f:
-            table = json.load(f)
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv"), newline="") as f:
+            rows = {r[0]: r for r in csv.reader(f)}
     except OSError:
         return None, None
-    e = table.get(f"{workload}/{maxleaf}/{precision}/{g_mode}")
-    return (e["dram_bytes"], e["source"]) if e else (None, None)
+    r = rows.get(f"{workload}/{maxleaf}/{precision}/{g_mode}")
+    return (float(r[1]), r[2]) if r else (None, None)
 
 
 def geometry(cfg):
@@ -612,7 +613,7 @@ def main(argv=None):
     ap.add_argument("--table-layout", default="paper", choices=["paper", "coef"])
     ap.add_argument("--softening-over-rcut", type=float, default=0.0)
     ap.add_argument("--warps-per-leaf", type=int, default=0)
-    ap.add_argument("--leaf-order", type=int, default=0, choices=[0, 1])
+    ap.add_argument("--leaf-order", type=int, default=0, choices=[0, 1], help="0 = ORB order (default), 1 = longest source list first")
     ap.add_argument("--maxleaf", type=int, default=0)
     ap.add_argument("--streams", type=int, default=1)
     ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")

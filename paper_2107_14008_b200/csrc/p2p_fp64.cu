@@ -44,7 +44,6 @@ struct P64Args {
     const double* table;      // TABLE: {T_i, E_i} pairs; COEF: TAB_STRIDE doubles per node; i = 0..tn
     int tn, tab_doubles;      // number of doubles to stage in shared memory
     double uk, h;             // u = r * uk in node units; h = 3 / tn
-    float hf;                 // (float) h
     void* out;                // caller order, n x 3
     int out_f32;
 };
@@ -102,19 +101,11 @@ __device__ __forceinline__ void g_eval(const P64Args& a, const double* __restric
             const double xi = fi[c] * a.h;                 // the node
             const double e = fma(r[c], a.inv2rs, -xi);     // eps = x - x_i, one rounding
             const double xi2 = xi * xi;
-            double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1)
-            if (LEVEL >= 3) {
-                // T[3] + T[4] are below (h/2)^2 = 1e-5 of T[1] + T[2]: their bracket e^2 (c_3 + e c_4) is evaluated in
-                // fp32 on the FMA pipe (relative error 1e-7 of a 1e-5 correction) and added once in fp64, which
-                // takes 5 instructions per pair off the FP64 pipe; T[1], T[2] and the sum stay in fp64.
-                const float xf = __int_as_float(0x4b000000 | idx[c]) - 8388608.0f;     // float(idx) without I2F
-                const float xif = xf * a.hf, xf2 = xif * xif, ef = (float)e;
-                float hi = fmaf(fmaf(xf2, 2.0f / 3.0f, -5.0f / 3.0f), xf2, 1.0f / 3.0f);
-                if (LEVEL >= 4) hi = fmaf(-xif * fmaf(fmaf(xf2, 1.0f / 3.0f, -1.5f), xf2, 1.0f), ef, hi);
-                poly = (double)(hi * ef * ef);
-            }
-            if (LEVEL >= 2) poly += fma(fma(-xi, xi2, xi), e, xi2);
-            else if (LEVEL >= 1) poly = xi2;
+            double poly = 0.0;   // sum_{k>=1} coefficient_k(x_i) e^(k-1), Horner from the highest kept level
+            if (LEVEL >= 4) poly = -xi * fma(fma(xi2, 1.0 / 3.0, -1.5), xi2, 1.0);
+            if (LEVEL >= 3) poly = fma(poly, e, fma(fma(xi2, 2.0 / 3.0, -5.0 / 3.0), xi2, 1.0 / 3.0));
+            if (LEVEL >= 2) poly = fma(poly, e, fma(-xi, xi2, xi));
+            if (LEVEL >= 1) poly = fma(poly, e, xi2);
             g[c] = LEVEL >= 1 ? fma(te.y * e, poly, te.x) : te.x;
         }
     }
@@ -336,7 +327,6 @@ int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool ou
         a.table = coef ? c->table.d_C64 : reinterpret_cast<const double*>(c->table.d_TE64);
         a.tab_doubles = (a.tn + 1) * (coef ? TAB_STRIDE : 2);
         a.h = 3.0 / a.tn;
-        a.hf = (float)a.h;
         a.uk = a.tn / 3.0 * a.inv2rs;
     }
     a.out = out; a.out_f32 = out_f32 ? 1 : 0;
