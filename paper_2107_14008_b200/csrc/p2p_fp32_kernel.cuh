@@ -11,7 +11,7 @@
 //   accumulation   fp32 per staged run, flushed into fp64 per-lane sums (two-level, A12)
 //   exact path     optional (close_pair_radius > 0): a staged run whose fp32 partial acceleration on a target exceeds
 //                  what one pair at close_pair_radius would give is re-evaluated in fp64 from the exact coordinates
-//                  for that target (nothing per pair in the fast path: three compares per run)
+//                  for that target by the whole warp (nothing per pair in the fast path: three compares per run)
 //   units          lengths in units of Ctx::pscale (a power of two near r_cut), G m in units of Ctx::gmscale (a power
 //                  of two >= max |G m|): exact rescalings that keep every fp32 intermediate in range whatever the
 //                  caller's units are; the fp64 sums are scaled back when they are stored
@@ -241,19 +241,23 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
 }
 
 // Exact path (A12): one target against one staged run of sources, in fp64 from the exact coordinates with
-// the library's erfc / exp — the oracle's arithmetic.  The lane's share of the run at e.x, exactly as the fast path
-// deals it out: source PAIRS first, first + step, ... (sources 2p and 2p + 1).  Returns the acceleration in caller units.
+// the library's erfc / exp — the oracle's arithmetic.  The whole warp works on it: the run's share of the target's owner
+// lane — source PAIRS first, first + step, ... (sources 2p and 2p + 1), exactly what the fast path dealt that lane — is
+// numbered m = 0, 1, ... and lane l takes m = l, l + 32, ...; the 32 partial sums are added in a fixed butterfly order,
+// so every lane returns the same, reproducible sum.  Returns the acceleration in caller units.
 // (scalars by value: a reference to the kernel's parameter block would make the compiler copy it to local memory)
 static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64, double Ld, double eps2_d, double rcut2_d,
                                                  double inv2rs_d, int tslot, uint2 e, int first, int step)
 {
+    const int lane = threadIdx.x & 31;
     const int ns = (int)(e.y & 0xffffu);
     const bool per_pair = (e.y & ENTRY_PER_PAIR) != 0;
     const double sx = Ld * ((int)((e.y >> 16) & 3u) - 1), sy = Ld * ((int)((e.y >> 18) & 3u) - 1), sz = Ld * ((int)((e.y >> 20) & 3u) - 1);
     const double4 pi = p64[tslot];
     double ax = 0, ay = 0, az = 0;
-    for (int jj = 2 * first; jj < ns; jj += 2 * step)
-    for (int j = jj; j < jj + 2; ++j) {
+    for (int m = lane;; m += 32) {
+        const int j = 2 * (first + step * (m >> 1)) + (m & 1);
+        if (j >= ns) break;
         const double4 pj = p64[e.x + j];
         double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (per_pair) {
@@ -269,6 +273,13 @@ static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64
             const double w = pj.w * (erfc(x) + 1.1283791670955125739 * x * exp(-x * x)) / (r2e * r);
             ax += w * dx; ay += w * dy; az += w * dz;
         }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ax += __shfl_xor_sync(0xffffffffu, ax, o);
+        ay += __shfl_xor_sync(0xffffffffu, ay, o);
+        az += __shfl_xor_sync(0xffffffffu, az, o);
     }
     return make_double3(ax, ay, az);
 }
@@ -498,10 +509,18 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : 1) p2p_fp32_kernel(P32Args a
         if (a.pth2 > 0.f) {
 #pragma unroll
             for (int t = 0; t < T; ++t) {
-                if (fmaf(px[t], px[t], fmaf(py[t], py[t], pz[t] * pz[t])) > a.pth2) {
-                    const double3 x = exact_run(a.p64, a.Ld, a.eps2_d, a.rcut2_d, a.inv2rs_d, tslot[t], e, half, pstep);
-                    ax[t] += x.x * a.inv_oscale; ay[t] += x.y * a.inv_oscale; az[t] += x.z * a.inv_oscale;
-                    px[t] = py[t] = pz[t] = 0.f;
+                const bool trig = fmaf(px[t], px[t], fmaf(py[t], py[t], pz[t] * pz[t])) > a.pth2;
+                unsigned todo = __ballot_sync(0xffffffffu, trig);
+                while (todo) {                       // warp-uniform: the warp redoes the run for one owner lane at a time
+                    const int owner = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    const int ts = __shfl_sync(0xffffffffu, tslot[t], owner);
+                    const int fo = HS > 1 ? owner / LG : 0;
+                    const double3 x = exact_run(a.p64, a.Ld, a.eps2_d, a.rcut2_d, a.inv2rs_d, ts, e, fo, pstep);
+                    if (lane == owner) {
+                        ax[t] += x.x * a.inv_oscale; ay[t] += x.y * a.inv_oscale; az[t] += x.z * a.inv_oscale;
+                        px[t] = py[t] = pz[t] = 0.f;
+                    }
                 }
             }
         }
