@@ -29,7 +29,7 @@ void free_leaves(Ctx* c)
 //     particles travel with the sort as float4 {x, y, z, caller index} in current order, so every pass reads
 //     and writes coalesced; the gather that applies the sorted order also reduces the children's bboxes.
 //   B (levels L0 .. depth-1): one CTA per level-L0 node finishes all remaining levels in shared memory
-//     (bitonic sorts on (child node, coordinate, local index) keys).
+//     (per level a radix select of every sub-node's median key and a stable partition about it).
 // Splitting coordinates are the positions rounded to fp32; ties go either way, which never changes `a`.
 
 constexpr int ORB_CTA_MAX = 4096;   // particles a phase-B CTA holds in shared memory
@@ -124,98 +124,191 @@ __global__ void orb_key_kernel(long long n, int level, const float4* __restrict_
     vals[q] = (uint32_t)q;
 }
 
-// sorts every aligned window of kmax keys ascending (kmax = n2: the whole array)
-template <typename Key>
-__device__ __forceinline__ void cta_bitonic_sort(Key* key, int n2, int kmax)
-{
-    for (int k = 2; k <= kmax; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = threadIdx.x; t < (n2 >> 1); t += blockDim.x) {
-                const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // the lower index of the t-th pair
-                const int l = i | j;
-                const Key a = key[i], b = key[l];
-                const bool up = (i & k) == 0 || k == kmax;
-                if ((a > b) == up) { key[i] = b; key[l] = a; }
-            }
-            __syncthreads();
-        }
-    }
-}
+// Phase B: CTA b owns the level-L0 node b, sorted positions [seg_start(L0, b), seg_start(L0, b + 1)), and finishes the
+// remaining levels in shared memory.  A level needs every sub-node split at its median along its widest axis - a stable
+// partition, not a sort: 24-bit fixed-point keys inside the sub-node's bbox, the median key by radix select (four
+// rounds of 6-bit digit histograms, one histogram per sub-node), then a stable partition about it (ballot ranks inside
+// a warp, one scan over the warps' totals).  Elements are dealt to the warps in blocks of 128 and to the lanes of a
+// warp round-robin, so every shared-memory access is lane-contiguous.
+constexpr int ORB_B_WARPS = ORB_CTA_THREADS / 32;
+constexpr int ORB_B_ITEMS = ORB_CTA_MAX / ORB_CTA_THREADS;      // 4 elements per thread
+constexpr int ORB_B_MAXSUB = 128;                               // sub-nodes of a CTA at its last level (4096 / 32, or / 16 ... / 2^7)
+constexpr int ORB_B_DIGIT = 6, ORB_B_BINS = 1 << ORB_B_DIGIT, ORB_B_ROUNDS = 4;   // 4 x 6 = 24 key bits
 
-// Phase B: CTA b owns the level-L0 node b, sorted positions [seg_start(L0, b), seg_start(L0, b + 1)).
+struct OrbBShared {
+    float4 cur[ORB_CTA_MAX];
+    unsigned hist[ORB_B_MAXSUB * ORB_B_BINS];
+    int blo[3 * ORB_B_MAXSUB], bhi[3 * ORB_B_MAXSUB];
+    unsigned prefix[ORB_B_MAXSUB], rank[ORB_B_MAXSUB], below[ORB_B_MAXSUB], ties[ORB_B_MAXSUB];
+    unsigned sbase[ORB_B_MAXSUB];            // packed (ties << 16 | less) before the sub-node's first element
+    int sstart[2][ORB_B_MAXSUB + 1];         // first element of each sub-node (this level / the next one)
+    unsigned wtot[ORB_B_WARPS], wbase[ORB_B_WARPS];
+};
+
 __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, int L0, int depth, const float4* __restrict__ P,
                                                                   uint32_t* __restrict__ perm)
 {
     extern __shared__ __align__(16) unsigned char orb_smem[];
+    OrbBShared& S = *reinterpret_cast<OrbBShared*>(orb_smem);
     const long long s0 = seg_start(n, L0, blockIdx.x);
     const long long s1 = blockIdx.x + 1 == (1LL << L0) ? n : seg_start(n, L0, blockIdx.x + 1);
     const int size = (int)(s1 - s0);
-    int n2 = 1;
-    while (n2 < size) n2 <<= 1;
-    unsigned long long* key = reinterpret_cast<unsigned long long*>(orb_smem);     // ORB_CTA_MAX
-    float4* cur = reinterpret_cast<float4*>(key + ORB_CTA_MAX);                    // ORB_CTA_MAX
-    int* blo = reinterpret_cast<int*>(cur + ORB_CTA_MAX);                          // 3 * 128
-    int* bhi = blo + 3 * 128;
-    for (int e = threadIdx.x; e < size; e += blockDim.x) cur[e] = P[s0 + e];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    // element r of this thread: warp-blocked, lane-striped
+    int el[ORB_B_ITEMS];
+#pragma unroll
+    for (int r = 0; r < ORB_B_ITEMS; ++r) el[r] = warp * (32 * ORB_B_ITEMS) + r * 32 + lane;
+#pragma unroll
+    for (int r = 0; r < ORB_B_ITEMS; ++r) if (el[r] < size) S.cur[el[r]] = P[s0 + el[r]];
+    if (threadIdx.x == 0) { S.sstart[0][0] = 0; S.sstart[0][1] = size; }
+    int sub[ORB_B_ITEMS];                            // sub-node of element el[r] at the current level
+#pragma unroll
+    for (int r = 0; r < ORB_B_ITEMS; ++r) sub[r] = 0;
     __syncthreads();
+
     for (int level = L0; level < depth; ++level) {
-        const int sl = level - L0;                   // nodes of this CTA at this level: 2^sl (<= 128)
+        const int sl = level - L0;                   // sub-nodes of this CTA at this level: 2^sl (<= ORB_B_MAXSUB)
         const int nsub = 1 << sl;
-        for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { blo[i] = 0x7fffffff; bhi[i] = (int)0x80000000; }
+        const int* sstart = S.sstart[sl & 1];
+        int* sstart_next = S.sstart[(sl + 1) & 1];
+        for (int i = threadIdx.x; i < 3 * nsub; i += blockDim.x) { S.blo[i] = 0x7fffffff; S.bhi[i] = (int)0x80000000; }
         __syncthreads();
-        for (int e0 = 0; e0 < size; e0 += blockDim.x) {       // whole warps enter: the votes below need all lanes
-            const int e = e0 + threadIdx.x;
-            const bool live = e < size;
-            const int sub = (int)seg_of(size, sl, live ? e : size - 1);
-            const float4 p = cur[live ? e : size - 1];
-            const int v[3] = {f2ord(p.x), f2ord(p.y), f2ord(p.z)};
-            const int sub0 = __shfl_sync(0xffffffffu, sub, 0);
-            if (__all_sync(0xffffffffu, sub == sub0)) {
+        float4 p[ORB_B_ITEMS];
+        // bounding boxes of the sub-nodes (whole warps enter: the votes need all lanes)
+#pragma unroll
+        for (int r = 0; r < ORB_B_ITEMS; ++r) {
+            const bool live = el[r] < size;
+            p[r] = S.cur[live ? el[r] : size - 1];
+            const int v[3] = {f2ord(p[r].x), f2ord(p[r].y), f2ord(p[r].z)};
+            const int sub0 = __shfl_sync(0xffffffffu, sub[r], 0);
+            if (__all_sync(0xffffffffu, sub[r] == sub0)) {
+#pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     const int mn = __reduce_min_sync(0xffffffffu, v[a]), mx = __reduce_max_sync(0xffffffffu, v[a]);
-                    if ((threadIdx.x & 31) == 0) { atomicMin(&blo[3 * sub + a], mn); atomicMax(&bhi[3 * sub + a], mx); }
+                    if (lane == 0) { atomicMin(&S.blo[3 * sub0 + a], mn); atomicMax(&S.bhi[3 * sub0 + a], mx); }
                 }
             } else if (live) {
-                for (int a = 0; a < 3; ++a) { atomicMin(&blo[3 * sub + a], v[a]); atomicMax(&bhi[3 * sub + a], v[a]); }
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { atomicMin(&S.blo[3 * sub[r] + a], v[a]); atomicMax(&S.bhi[3 * sub[r] + a], v[a]); }
             }
         }
+        for (int k = threadIdx.x; k < nsub; k += blockDim.x) {
+            S.prefix[k] = 0; S.below[k] = 0;
+            S.rank[k] = (unsigned)((sstart[k + 1] - sstart[k]) >> 1);    // first element of the right child
+        }
         __syncthreads();
-        // A node that holds a power of two of particles has its sub-nodes in aligned windows: they are sorted
-        // separately (fewer bitonic stages) on 32-bit keys (coordinate quantised to 20 bits inside the sub-node's
-        // bbox | local index).  Any other size: one sort of 64-bit keys (sub-node | fp32 coordinate | local index).
-        const bool windowed = size == n2;
-        unsigned* key32 = reinterpret_cast<unsigned*>(key);
-        for (int e = threadIdx.x; e < n2; e += blockDim.x) {
-            unsigned long long k = ~0ULL;            // padding sorts to the end
-            if (e < size) {
-                const int sub = (int)seg_of(size, sl, e);
-                float lo3[3], ext[3];
-                for (int a = 0; a < 3; ++a) { lo3[a] = ord2f(blo[3 * sub + a]); ext[a] = ord2f(bhi[3 * sub + a]) - lo3[a]; }
-                const int axis = widest_axis(ext);
-                const float4 p = cur[e];
-                const float x = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
-                if (windowed) {
-                    const float u = ext[axis] > 0.f ? (x - lo3[axis]) / ext[axis] : 0.f;
-                    k = ((unsigned)fminf(u * 1048575.0f, 1048575.0f) << 12) | (unsigned)e;
-                } else {
-                    k = ((unsigned long long)sub << 44) | ((unsigned long long)((unsigned)f2ord(x) ^ 0x80000000u) << 12) | (unsigned)e;
+        // keys: coordinate along the sub-node's widest axis as a 24-bit fixed-point number inside its bbox
+        unsigned key[ORB_B_ITEMS];
+#pragma unroll
+        for (int r = 0; r < ORB_B_ITEMS; ++r) {
+            float lo3[3], ext[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { lo3[a] = ord2f(S.blo[3 * sub[r] + a]); ext[a] = ord2f(S.bhi[3 * sub[r] + a]) - lo3[a]; }
+            const int axis = widest_axis(ext);
+            const float x = axis == 0 ? p[r].x : axis == 1 ? p[r].y : p[r].z;
+            const float u = ext[axis] > 0.f ? (x - lo3[axis]) / ext[axis] : 0.f;
+            key[r] = (unsigned)fminf(u * 16777215.0f, 16777215.0f);
+        }
+        // median key of every sub-node by radix select
+        for (int round = 0; round < ORB_B_ROUNDS; ++round) {
+            const int shift = ORB_B_DIGIT * (ORB_B_ROUNDS - 1 - round);
+            for (int i = threadIdx.x; i < nsub * ORB_B_BINS; i += blockDim.x) S.hist[i] = 0;
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < ORB_B_ITEMS; ++r) {
+                if (el[r] < size && (round == 0 || (key[r] >> (shift + ORB_B_DIGIT)) == S.prefix[sub[r]]))
+                    atomicAdd(&S.hist[sub[r] * ORB_B_BINS + ((key[r] >> shift) & (ORB_B_BINS - 1))], 1u);
+            }
+            __syncthreads();
+            for (int k = warp; k < nsub; k += ORB_B_WARPS) {       // one warp per sub-node: the bin that holds the rank
+                const unsigned v0 = S.hist[k * ORB_B_BINS + 2 * lane], v1 = S.hist[k * ORB_B_BINS + 2 * lane + 1];
+                const unsigned s = v0 + v1;
+                unsigned inc = s;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                const unsigned rk = S.rank[k];
+                const unsigned cum = inc - s;
+                int bin = -1;
+                unsigned cb = 0, hb = 0;
+                if (rk >= cum && rk < cum + v0) { bin = 2 * lane; cb = cum; hb = v0; }
+                else if (rk >= cum + v0 && rk < cum + s) { bin = 2 * lane + 1; cb = cum + v0; hb = v1; }
+                const unsigned owner = __ballot_sync(0xffffffffu, bin >= 0);
+                if (owner && lane == __ffs(owner) - 1) {           // exactly one lane (rank < size of the sub-node)
+                    S.prefix[k] = (S.prefix[k] << ORB_B_DIGIT) | (unsigned)bin;
+                    S.rank[k] = rk - cb;
+                    S.below[k] += cb;
+                    S.ties[k] = hb;
                 }
             }
-            if (windowed) key32[e] = (unsigned)k;
-            else key[e] = k;
+            __syncthreads();
+        }
+        // stable partition of every sub-node about its median key m: keys < m and the first (left - #less) keys == m
+        // go left, the rest right, each side in its old order
+        unsigned ex[ORB_B_ITEMS];
+        {
+            unsigned run = 0;                         // packed (ties << 16 | less) of this warp's elements so far
+#pragma unroll
+            for (int r = 0; r < ORB_B_ITEMS; ++r) {
+                const bool live = el[r] < size;
+                const unsigned m = S.prefix[sub[r]];
+                const unsigned bl = __ballot_sync(0xffffffffu, live && key[r] < m);
+                const unsigned bt = __ballot_sync(0xffffffffu, live && key[r] == m);
+                ex[r] = run + (unsigned)__popc(bl & lt_mask) + ((unsigned)__popc(bt & lt_mask) << 16);
+                run += (unsigned)__popc(bl) + ((unsigned)__popc(bt) << 16);
+            }
+            if (lane == 0) S.wtot[warp] = run;
         }
         __syncthreads();
-        if (windowed) cta_bitonic_sort(key32, n2, n2 >> sl);
-        else cta_bitonic_sort(key, n2, n2);
-        // apply the order: read through the sorted local indices, then write back
-        float4 tmp[ORB_CTA_MAX / ORB_CTA_THREADS];
-        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r)
-            tmp[r] = cur[windowed ? (int)(key32[e] & 0xfffu) : (int)(key[e] & 0xfffu)];
+        if (warp == 0) {
+            const unsigned v = S.wtot[lane];
+            unsigned inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            S.wbase[lane] = inc - v;
+        }
         __syncthreads();
-        for (int e = threadIdx.x, r = 0; e < size; e += blockDim.x, ++r) cur[e] = tmp[r];
+#pragma unroll
+        for (int r = 0; r < ORB_B_ITEMS; ++r) {
+            ex[r] += S.wbase[warp];
+            if (el[r] < size && el[r] == sstart[sub[r]]) S.sbase[sub[r]] = ex[r];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < ORB_B_ITEMS; ++r) {
+            if (el[r] >= size) { sub[r] = 2 * nsub - 1; continue; }     // padding follows the last element
+            const int k = sub[r];
+            const int st = sstart[k];
+            const unsigned left = (unsigned)((sstart[k + 1] - st) >> 1);
+            const unsigned m = S.prefix[k], less_total = S.below[k], tie_total = S.ties[k];
+            const unsigned need = left - less_total;                 // ties that still go left
+            const unsigned rel = ex[r] - S.sbase[k];                 // both fields are >= the base's: no borrow
+            const unsigned lb = rel & 0xffffu, tb = rel >> 16;
+            const unsigned idx = (unsigned)(el[r] - st);
+            unsigned dst;
+            if (key[r] < m) dst = lb;
+            else if (key[r] == m) dst = tb < need ? less_total + tb : left + (tb - need);
+            else dst = left + (tie_total - need) + (idx - lb - tb);
+            S.cur[st + (int)dst] = p[r];
+            sub[r] = 2 * k + (el[r] - st >= (int)left);       // the sub-node of POSITION el[r] one level down
+        }
+        for (int k = threadIdx.x; k < nsub; k += blockDim.x) {
+            const int st = sstart[k];
+            sstart_next[2 * k] = st;
+            sstart_next[2 * k + 1] = st + ((sstart[k + 1] - st) >> 1);
+            if (k == nsub - 1) sstart_next[2 * nsub] = size;
+        }
         __syncthreads();
     }
-    for (int e = threadIdx.x; e < size; e += blockDim.x) perm[s0 + e] = (uint32_t)__float_as_int(cur[e].w);
+#pragma unroll
+    for (int r = 0; r < ORB_B_ITEMS; ++r)
+        if (el[r] < size) perm[s0 + el[r]] = (uint32_t)__float_as_int(S.cur[el[r]].w);
 }
 
 // ------------------------------------------------------------------------------ leaf table + packing
@@ -319,8 +412,9 @@ struct ListArgs {
 
 __global__ void list_kernel(ListArgs a)
 {
-    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= a.n_leaves) return;
+    const long long i_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const bool live = i_raw < a.n_leaves;
+    const long long i = live ? i_raw : a.n_leaves - 1;
     const int leaf0 = (int)(a.n_leaves - 1);   // heap index of leaf 0
     // fp32 walk on {centre, half-width} boxes whose half-widths were rounded up (node_box32_kernel) and with a
     // slack of 1e-6 L on every gap: it can only accept more than the exact test would, never less.
@@ -330,20 +424,27 @@ __global__ void list_kernel(ListArgs a)
     const float amb = Lf - 2.0f * (float)a.rcut;      // ambiguous image iff 2 (hw_i + hw_j) >= amb  (A10)
     const int my_cnt = a.leaf_cnt[i];
 
-    int stack[40];
-    int sp = 0;
-    stack[sp++] = 0;
-    long long run_first = -1, run_n = 0, n_chunks = 0, n_pairs = 0, n_eval = 0, work = 0;
-    int run_code = -1;
+    int run_first = -1, run_n = 0, run_code = -1, n_chunks = 0, n_pairs = 0;
+    long long n_eval = 0;
     // Pass 1 counts and keeps the first stash_cap entries of every leaf; pass 2 (only the leaves whose list
     // did not fit, the rest is a plain copy by list_copy_kernel) walks again and writes in place.
-    if (a.chunks && a.n_chunks_of[i] <= a.stash_cap) return;
+    const bool skip = !live || (a.chunks && a.n_chunks_of[i] <= a.stash_cap);
     uint2* out = a.chunks ? a.chunks + a.chunk_ptr[i] : nullptr;
     uint2* stash = a.chunks ? nullptr : a.stash + i * a.stash_cap;
     const int max_leaves_per_chunk = a.chunk_max / a.maxleaf;
+    auto emit = [&]() {
+        const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
+        if (out) out[n_chunks] = ent;
+        else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
+        ++n_chunks;
+    };
 
-    while (sp) {
-        const int node = stack[--sp];
+    // Stackless depth-first walk of the complete binary tree: with 1-based heap indices the children of h are 2h and
+    // 2h + 1, and the node that follows the subtree of h is (h + 1) >> ctz(h + 1) (up while h is a right child, then
+    // on to the sibling); arriving at 1 = back at the root = done.  Left child first: leaves come out in ascending order.
+    unsigned h = skip ? 0u : 1u;
+    while (h) {
+        const int node = (int)h - 1;
         const float4 nc = __ldg(&a.box[2 * (size_t)node]), nhw = __ldg(&a.box[2 * (size_t)node + 1]);
         float g2 = 0.f;
         int code = 0;                 // the three shift fields of entry_pack, without the slot count
@@ -361,41 +462,40 @@ __global__ void list_kernel(ListArgs a)
                 if (a.periodic && 2.0f * hws[x] >= amb) ambiguous = true;
             }
         }
-        if (!(g2 < rc2)) continue;
-        if (node < leaf0) {               // internal: right child first so the left one is popped first
-            stack[sp++] = 2 * node + 2;
-            stack[sp++] = 2 * node + 1;
-            continue;
-        }
-        const long long j = node - leaf0;
-        if (ambiguous) code = (int)entry_pack(0, 0, 0, 0, true);
-        ++n_pairs;
-        n_eval += (long long)my_cnt * a.leaf_cnt[j];
-        work += a.maxleaf;
-        if (run_n > 0 && j == run_first + run_n && code == run_code && run_n < max_leaves_per_chunk) {
-            ++run_n;
-        } else {
-            if (run_n > 0) {
-                const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
-                if (out) out[n_chunks] = ent;
-                else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
-                ++n_chunks;
+        const bool accept = g2 < rc2;
+        if (accept && node < leaf0) { h = 2 * h; continue; }       // internal: down to the left child
+        if (accept) {
+            const int j = node - leaf0;
+            if (ambiguous) code = (int)entry_pack(0, 0, 0, 0, true);
+            ++n_pairs;
+            n_eval += (long long)my_cnt * a.leaf_cnt[j];
+            if (run_n > 0 && j == run_first + run_n && code == run_code && run_n < max_leaves_per_chunk) {
+                ++run_n;
+            } else {
+                if (run_n > 0) emit();
+                run_first = j; run_n = 1; run_code = code;
             }
-            run_first = j; run_n = 1; run_code = code;
         }
+        const unsigned up = h + 1;
+        h = up >> (__ffs(up) - 1);
+        if (h == 1) h = 0;
     }
-    if (run_n > 0) {
-        const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
-        if (out) out[n_chunks] = ent;
-        else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
-        ++n_chunks;
-    }
-    if (!a.chunks) {
-        a.n_chunks_of[i] = n_chunks;
-        a.work_of[i] = work;
-        atomicAdd(&a.totals[0], (unsigned long long)n_pairs);
-        atomicAdd(&a.totals[1], (unsigned long long)n_eval);
-        atomicMax(&a.totals[2], (unsigned long long)work);
+    if (run_n > 0) emit();
+    if (!a.chunks) {       // whole warps arrive here
+        const long long work = (long long)n_pairs * a.maxleaf;
+        if (live) { a.n_chunks_of[i] = n_chunks; a.work_of[i] = work; }
+        unsigned long long tp = (unsigned long long)n_pairs, te = (unsigned long long)n_eval, tw = (unsigned long long)work;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            tp += __shfl_xor_sync(0xffffffffu, tp, o);
+            te += __shfl_xor_sync(0xffffffffu, te, o);
+            tw = max(tw, __shfl_xor_sync(0xffffffffu, tw, o));
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(&a.totals[0], tp);
+            atomicAdd(&a.totals[1], te);
+            atomicMax(&a.totals[2], tw);
+        }
     }
 }
 
@@ -526,7 +626,8 @@ static int orb_sort(Ctx* c, int depth, cudaStream_t st)
         }
     }
     if (depth > L0) {
-        const size_t smem = (size_t)ORB_CTA_MAX * (8 + 16) + 2 * 3 * 128 * sizeof(int);
+        const size_t smem = sizeof(OrbBShared);
+        if (depth - L0 > 8) return fail(c, PHOTONS_EINVAL, "build_leaves: more than 8 ORB levels below a 4096-particle node");
         PH_CUDA_BUILD(cudaFuncSetAttribute(orb_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         orb_cta_kernel<<<(unsigned)(1LL << L0), ORB_CTA_THREADS, smem, st>>>(n, L0, depth, P_cur, c->d_perm);
     } else {

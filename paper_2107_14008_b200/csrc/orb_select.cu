@@ -180,15 +180,19 @@ __global__ void __launch_bounds__(256) sel_scan_kernel(SelLevel L, const uint2* 
     }
 }
 
-// 5. stable partition of every node about its median key; child bounding boxes on the way (lo2 == nullptr: not needed)
+// 5. stable partition of every node about its median key; child bounding boxes on the way (lo2 == nullptr: not needed).
+// A chunk is dealt to its 8 warps in blocks of 256 elements and to the lanes of a warp round-robin: loads are
+// lane-contiguous, ranks inside a warp come from ballots, and the lanes that go to the same side store to consecutive
+// addresses.  The boxes are reduced over the whole CTA (a chunk lies inside one node) before the global atomics.
 __global__ void __launch_bounds__(SEL_THREADS) sel_scatter_kernel(SelLevel L, long long n, const float4* __restrict__ P,
                                                                   const unsigned* __restrict__ keys, const unsigned* __restrict__ median,
                                                                   const unsigned* __restrict__ below, const unsigned* __restrict__ ties,
                                                                   const uint2* __restrict__ ch_base, float4* __restrict__ P_out,
                                                                   int* __restrict__ lo2, int* __restrict__ hi2)
 {
-    typedef cub::BlockScan<unsigned, SEL_THREADS> Scan;
-    __shared__ typename Scan::TempStorage tmp;
+    constexpr int NW = SEL_THREADS / 32;
+    __shared__ unsigned wtot[NW];
+    __shared__ int s_mn[NW][6], s_mx[NW][6];
     const int c = blockIdx.x, node = L.ch_node[c], cnt = L.ch_cnt[c];
     const long long q0 = L.ch_q0[c];
     const long long s0 = seg_start(n, L.level, node), s1 = node + 1 == L.n_nodes ? n : seg_start(n, L.level, node + 1);
@@ -196,18 +200,26 @@ __global__ void __launch_bounds__(SEL_THREADS) sel_scatter_kernel(SelLevel L, lo
     const unsigned m = median[node], less_total = below[node], tie_total = ties[node];
     const unsigned need = left - less_total;          // ties that still go left
     const uint2 base = ch_base[c];
-    const int e0 = threadIdx.x * SEL_ITEMS;           // this thread's SEL_ITEMS consecutive elements: order is kept
-    unsigned k[SEL_ITEMS];
-    unsigned nl = 0, nt = 0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const int e0 = warp * (32 * SEL_ITEMS) + lane;    // element i of this thread: e0 + 32 i
+    unsigned k[SEL_ITEMS], ex[SEL_ITEMS];
+    float4 p[SEL_ITEMS];
+    unsigned run = 0;                                 // packed (ties << 16 | less) of this warp's elements so far
 #pragma unroll
     for (int i = 0; i < SEL_ITEMS; ++i) {
-        k[i] = e0 + i < cnt ? keys[q0 + e0 + i] : 0xffffffffu;
-        nl += k[i] < m;
-        nt += k[i] == m;
+        const int e = e0 + 32 * i;
+        const bool live = e < cnt;
+        k[i] = live ? keys[q0 + e] : 0xffffffffu;
+        if (live) p[i] = P[q0 + e];
+        const unsigned bl = __ballot_sync(0xffffffffu, k[i] < m), bt = __ballot_sync(0xffffffffu, k[i] == m);
+        ex[i] = run + (unsigned)__popc(bl & lt_mask) + ((unsigned)__popc(bt & lt_mask) << 16);
+        run += (unsigned)__popc(bl) + ((unsigned)__popc(bt) << 16);
     }
-    unsigned packed = (nt << 16) | nl, ex;            // at most 2048 of each per chunk
-    Scan(tmp).ExclusiveSum(packed, ex);
-    unsigned lb = base.x + (ex & 0xffffu), tb = base.y + (ex >> 16);     // less / tie elements of this node before mine
+    if (lane == 0) wtot[warp] = run;
+    __syncthreads();
+    unsigned wb = 0;
+    for (int w = 0; w < warp; ++w) wb += wtot[w];
     int mn[2][3], mx[2][3];
 #pragma unroll
     for (int s = 0; s < 2; ++s)
@@ -215,24 +227,23 @@ __global__ void __launch_bounds__(SEL_THREADS) sel_scatter_kernel(SelLevel L, lo
         for (int a = 0; a < 3; ++a) { mn[s][a] = 0x7fffffff; mx[s][a] = (int)0x80000000; }
 #pragma unroll
     for (int i = 0; i < SEL_ITEMS; ++i) {
-        if (e0 + i >= cnt) break;
-        const long long q = q0 + e0 + i;
-        const unsigned idx = (unsigned)(q - s0);      // position inside the node
-        long long dst;
+        const int e = e0 + 32 * i;
+        if (e >= cnt) continue;
+        const unsigned rel = ex[i] + wb;
+        const unsigned lb = base.x + (rel & 0xffffu), tb = base.y + (rel >> 16);   // less / tie elements of this node before mine
+        const unsigned idx = (unsigned)(q0 + e - s0);     // position inside the node
+        unsigned dst;
         int side;
-        if (k[i] < m) { dst = s0 + lb; ++lb; side = 0; }
+        if (k[i] < m) { dst = lb; side = 0; }
         else if (k[i] == m) {
-            if (tb < need) { dst = s0 + less_total + tb; side = 0; }
-            else { dst = s0 + left + (tb - need); side = 1; }
-            ++tb;
+            if (tb < need) { dst = less_total + tb; side = 0; }
+            else { dst = left + (tb - need); side = 1; }
         } else {
-            const unsigned gb = idx - (lb + tb);      // greater elements before mine
-            dst = s0 + left + (tie_total - need) + gb;
+            dst = left + (tie_total - need) + (idx - (lb + tb));      // greater elements before mine
             side = 1;
         }
-        const float4 p = P[q];
-        P_out[dst] = p;
-        const int v[3] = {f2ord(p.x), f2ord(p.y), f2ord(p.z)};
+        P_out[s0 + dst] = p[i];
+        const int v[3] = {f2ord(p[i].x), f2ord(p[i].y), f2ord(p[i].z)};
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             if (side == 0) { mn[0][a] = min(mn[0][a], v[a]); mx[0][a] = max(mx[0][a], v[a]); }
@@ -245,11 +256,17 @@ __global__ void __launch_bounds__(SEL_THREADS) sel_scatter_kernel(SelLevel L, lo
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             const int wmn = __reduce_min_sync(0xffffffffu, mn[s][a]), wmx = __reduce_max_sync(0xffffffffu, mx[s][a]);
-            if ((threadIdx.x & 31) == 0 && wmn <= wmx) {
-                atomicMin(&lo2[3 * (2 * (size_t)node + s) + a], wmn);
-                atomicMax(&hi2[3 * (2 * (size_t)node + s) + a], wmx);
-            }
+            if (lane == 0) { s_mn[warp][3 * s + a] = wmn; s_mx[warp][3 * s + a] = wmx; }
         }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        int bmn = s_mn[0][threadIdx.x], bmx = s_mx[0][threadIdx.x];
+        for (int w = 1; w < NW; ++w) { bmn = min(bmn, s_mn[w][threadIdx.x]); bmx = max(bmx, s_mx[w][threadIdx.x]); }
+        if (bmn <= bmx) {                              // threadIdx.x = 3 side + axis
+            atomicMin(&lo2[6 * (size_t)node + threadIdx.x], bmn);
+            atomicMax(&hi2[6 * (size_t)node + threadIdx.x], bmx);
+        }
+    }
 }
 
 __global__ void sel_fill_kernel(long long n, int* p, int v)

@@ -232,6 +232,46 @@ def test_pairs_evaluated_and_list_cover(B, c1):
     assert set(np.unique(code)) <= set(range(28))
 
 
+@pytest.mark.parametrize("n,maxleaf,clustered", [(32768, 32, False), (20011, 16, False), (5000, 64, False), (262144, 32, True),
+                                                 (100003, 32, True)])
+def test_orb_tree_is_a_median_split_along_the_widest_axis(B, n, maxleaf, clustered):
+    """PAPER.md L35 / DESIGN.md A13, checked on the device-built tree itself: every node is cut along the widest axis of
+    its particle bounding box (fp32 coordinates), the left child takes floor(size/2) particles and no particle of the
+    left child lies beyond one of the right child (up to the 24-bit key quantum of the partition, ties either way).
+    Covers both build phases: nodes above 4096 particles (global partition passes) and below (shared memory)."""
+    rng = np.random.default_rng(77)
+    if clustered:
+        cen = rng.random((40, 3))
+        pos = (cen[rng.integers(0, 40, n)] + 0.01 * rng.standard_normal((n, 3)) * rng.random((n, 1)) ** 3) % 1.0
+        pos[: n // 5] = rng.random((n // 5, 3))
+    else:
+        pos = rng.random((n, 3))
+    pos = pos.astype(np.float32).astype(np.float64)
+    mass = np.full(n, 1.0 / n)
+    with B.Photons(n_pm=32, maxleaf=maxleaf, precision="fp64", g_mode="direct") as ph:
+        ph.set_particles(pos, mass)
+        ph.build_leaves()
+        perm, leaf_start = ph.leaf_order()
+    assert np.array_equal(np.sort(perm), np.arange(n))
+    n_leaves = len(leaf_start) - 1
+    depth = int(np.log2(n_leaves))
+    assert 1 << depth == n_leaves and np.diff(leaf_start).max() <= maxleaf
+    x = pos[perm]
+    for level in range(depth):
+        step = n_leaves >> level
+        bounds = leaf_start[::step]
+        for k in range(1 << level):
+            s0, s1 = int(bounds[k]), int(bounds[k + 1])
+            mid = int(leaf_start[k * step + step // 2])
+            assert mid - s0 == (s1 - s0) // 2
+            node = x[s0:s1]
+            ext = node.max(axis=0) - node.min(axis=0)
+            axis = int(np.argmax(ext))              # ties -> lowest axis, as A13
+            left, right = x[s0:mid, axis], x[mid:s1, axis]
+            if len(left) and len(right):
+                assert left.max() <= right.min() + ext[axis] * 2.0 ** -20, (level, k, axis)
+
+
 # ------------------------------------------------------------------- ragged sizes and degenerate cases
 
 @pytest.mark.parametrize("n", [1, 2, 3, 31, 33, 100, 1000, 5000, 20011])
