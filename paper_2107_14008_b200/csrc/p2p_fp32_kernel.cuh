@@ -24,7 +24,15 @@
                               // 2: 103.2 ms, 4: 96.3 ms, 8: 94.4 ms)
 #endif
 #ifndef PHOTONS_UNROLL_T2
-#define PHOTONS_UNROLL_T2 2   // ... with two targets per lane
+#define PHOTONS_UNROLL_T2 4   // ... with two targets per lane (MAXLEAF 64 on config 4: 2: 122.0 ms, 4 with two CTAs of 256 per SM: 119.6 ms)
+#endif
+#ifndef PHOTONS_PRED_ACC
+#define PHOTONS_PRED_ACC 1    // two targets per lane, full-warp groups: the cut as a predicate on scalar accumulation FFMAs
+                              // instead of a select on the weight (config 4, MAXLEAF 64: 117.3 against 119.6 ms; with one target
+                              // per lane it changes nothing at MAXLEAF 32 and costs 3 % at MAXLEAF 16, so it stays off there)
+#endif
+#ifndef PHOTONS_MINBLOCKS_T2
+#define PHOTONS_MINBLOCKS_T2 2   // __launch_bounds__(256, .) of the kernels with two targets per lane
 #endif
 
 namespace photons {
@@ -185,7 +193,8 @@ struct LoopConst {
     float tk, rcut2, r2add, ek, tmap, inv2rs;
 };
 
-template <int GKIND, int GPAR, int NCH>
+// SEL = false: the cut is left to the caller (acc_cut below), w is the raw value
+template <int GKIND, int GPAR, int NCH, bool SEL>
 __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, const float2* tab, const float2 (&r2)[NCH],
                                         const float2 (&gm)[NCH], float2 (&w)[NCH])
 {
@@ -207,7 +216,7 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
             const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
             const float2 u = __ffma2_rn(idr2, idr[c], f2(-q[c].x, -q[c].y));
             const float2 v = __fmul2_rn(u, gm[c]);
-            w[c] = f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f);
+            w[c] = SEL ? f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f) : v;
         }
     } else if (GKIND == GM_FUSED) {
         // Eq. 1 evaluated directly, hand-fused: g = exp(-x^2) H(x) with H = erfcx(x) + 2x/sqrt(pi), smooth on [0, 3]:
@@ -232,12 +241,22 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
         for (int c = 0; c < NCH; ++c) {
             const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
             const float2 v = __fmul2_rn(__fmul2_rn(q[c], e[c]), __fmul2_rn(idr2, __fmul2_rn(idr[c], gm[c])));
-            w[c] = f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f);
+            w[c] = SEL ? f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f) : v;
         }
     } else {
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR>(a, tab, r2[c], gm[c]);
+        for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR>(a, tab, r2[c], gm[c]);    // (selects inside)
     }
+}
+
+// The cut (A8) as a predicate on the accumulation: acc += w d iff r2 < rcut2 - one FSETP and three predicated scalar
+// FFMAs per pair, against FSETP + FSEL and 1.5 FFMA2: the same FMA-pipe time and one issue slot less.  A w that is
+// Inf/NaN far outside the approximation's range is never touched.
+__device__ __forceinline__ void acc_cut(float& ax, float& ay, float& az, float w, float dx, float dy, float dz, float r2, float rcut2)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f32 p, %7, %8;\n\t@p fma.rn.f32 %0, %3, %4, %0;\n\t@p fma.rn.f32 %1, %3, %5, %1;\n\t"
+        "@p fma.rn.f32 %2, %3, %6, %2;\n\t}"
+        : "+f"(ax), "+f"(ay), "+f"(az) : "f"(w), "f"(dx), "f"(dy), "f"(dz), "f"(r2), "f"(rcut2));
 }
 
 // Exact path (A12): one target against one staged run of sources, in fp64 from the exact coordinates with
@@ -287,7 +306,7 @@ static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64
 // ---------------------------------------------------------------------------------------------------------
 
 template <int T, int HS, bool MIXED, int GKIND, int GPAR>
-__global__ void __launch_bounds__(256, T == 1 ? 3 : 1) p2p_fp32_kernel(P32Args a)
+__global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T2 : 1) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
@@ -459,7 +478,8 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : 1) p2p_fp32_kernel(P32Args a
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
                 // U source pairs x T targets = NCH independent chains per iteration
                 // (with lane groups the leaf's np = maxleaf/2 source pairs are shared out, so fewer fit in one iteration)
-                constexpr int U = T == 1 ? (HS == 1 ? PHOTONS_UNROLL_T1 : PHOTONS_UNROLL_T1 / 2) : T == 2 ? PHOTONS_UNROLL_T2 : 1;
+                constexpr int U = T == 1 ? (HS == 1 ? PHOTONS_UNROLL_T1 : PHOTONS_UNROLL_T1 / 2) : T == 2 ? (HS == 4 ? 2 : PHOTONS_UNROLL_T2) : 1;
+                static_assert(U * HS <= 16 * T / HS, "a leaf's source pairs must fill whole iterations");
                 constexpr int NCH = U * T;
                 auto step = [&](const int p, const bool with_seam) {
                     float2 dx[NCH], dy[NCH], dz[NCH], r2[NCH], gm[NCH], w[NCH];
@@ -479,15 +499,21 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : 1) p2p_fp32_kernel(P32Args a
                     for (int c = 0; c < NCH; ++c) {
                         r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(kc.r2add))));
                     }
-                    weights<GKIND, GPAR, NCH>(a, kc, tab, r2, gm, w);
+                    constexpr bool PRED = PHOTONS_PRED_ACC && T == 2 && HS == 1 && (GKIND == GM_POLY || GKIND == GM_FUSED);
+                    weights<GKIND, GPAR, NCH, !PRED>(a, kc, tab, r2, gm, w);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
 #pragma unroll
                         for (int t = 0; t < T; ++t) {
                             const int c = u * T + t;
-                            pax[t] = __ffma2_rn(w[c], dx[c], pax[t]);
-                            pay[t] = __ffma2_rn(w[c], dy[c], pay[t]);
-                            paz[t] = __ffma2_rn(w[c], dz[c], paz[t]);
+                            if (PRED) {
+                                acc_cut(pax[t].x, pay[t].x, paz[t].x, w[c].x, dx[c].x, dy[c].x, dz[c].x, r2[c].x, kc.rcut2);
+                                acc_cut(pax[t].y, pay[t].y, paz[t].y, w[c].y, dx[c].y, dy[c].y, dz[c].y, r2[c].y, kc.rcut2);
+                            } else {
+                                pax[t] = __ffma2_rn(w[c], dx[c], pax[t]);
+                                pay[t] = __ffma2_rn(w[c], dy[c], pay[t]);
+                                paz[t] = __ffma2_rn(w[c], dz[c], paz[t]);
+                            }
                         }
                     }
                 };
