@@ -446,27 +446,24 @@ __global__ void list_kernel(ListArgs a)
     while (h) {
         const int node = (int)h - 1;
         const float4 nc = __ldg(&a.box[2 * (size_t)node]), nhw = __ldg(&a.box[2 * (size_t)node + 1]);
+        // periodic bbox-to-bbox distance (A11): per axis the nearest image of the centre difference, less the half-widths
+        const float dcs[3] = {nc.x - tc.x, nc.y - tc.y, nc.z - tc.z};
+        const float hws[3] = {nhw.x + thw.x, nhw.y + thw.y, nhw.z + thw.z};
+        float img[3];                 // the source is moved by -img box lengths
         float g2 = 0.f;
-        int code = 0;                 // the three shift fields of entry_pack, without the slot count
-        bool ambiguous = false;
-        {
-            const float dcs[3] = {nc.x - tc.x, nc.y - tc.y, nc.z - tc.z};
-            const float hws[3] = {nhw.x + thw.x, nhw.y + thw.y, nhw.z + thw.z};
 #pragma unroll
-            for (int x = 0; x < 3; ++x) {
-                const float img = a.periodic ? rintf(dcs[x] * invL) : 0.f;      // source is moved by -img box lengths
-                const float dc = fmaf(-Lf, img, dcs[x]);
-                const float gap = fmaxf(0.f, fabsf(dc) - hws[x] - slack);
-                g2 = fmaf(gap, gap, g2);
-                code |= (1 - (int)img) << (16 + 2 * x);
-                if (a.periodic && 2.0f * hws[x] >= amb) ambiguous = true;
-            }
+        for (int x = 0; x < 3; ++x) {
+            img[x] = a.periodic ? rintf(dcs[x] * invL) : 0.f;
+            const float gap = fmaxf(0.f, fabsf(fmaf(-Lf, img[x], dcs[x])) - (hws[x] + slack));
+            g2 = fmaf(gap, gap, g2);
         }
         const bool accept = g2 < rc2;
         if (accept && node < leaf0) { h = 2 * h; continue; }       // internal: down to the left child
         if (accept) {
             const int j = node - leaf0;
-            if (ambiguous) code = (int)entry_pack(0, 0, 0, 0, true);
+            // the three shift fields of entry_pack, without the slot count; ambiguous image -> per-pair flag (A10)
+            int code = ((1 - (int)img[0]) << 16) | ((1 - (int)img[1]) << 18) | ((1 - (int)img[2]) << 20);
+            if (a.periodic && 2.0f * fmaxf(hws[0], fmaxf(hws[1], hws[2])) >= amb) code = (int)entry_pack(0, 0, 0, 0, true);
             ++n_pairs;
             n_eval += (long long)my_cnt * a.leaf_cnt[j];
             if (run_n > 0 && j == run_first + run_n && code == run_code && run_n < max_leaves_per_chunk) {
