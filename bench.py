@@ -281,6 +281,8 @@ def run_ours(args):
         params["warps_per_leaf"] = args.warps_per_leaf
     if args.targets_per_lane:
         params["targets_per_lane"] = args.targets_per_lane
+    if args.chunk_max:
+        params["chunk_max"] = args.chunk_max
     if args.leaf_order:
         params["leaf_order"] = args.leaf_order
     if args.no_close or args.precision == "fp64":
@@ -615,6 +617,7 @@ def main(argv=None):
     ap.add_argument("--table-layout", default="paper", choices=["paper", "coef"])
     ap.add_argument("--softening-over-rcut", type=float, default=0.0)
     ap.add_argument("--warps-per-leaf", type=int, default=0)
+    ap.add_argument("--chunk-max", type=int, default=0, help="longest staged run in source slots (0 = the library default)")
     ap.add_argument("--targets-per-lane", type=int, default=0, help="register tiling of the fp32 kernels (0 = the default of the leaf size)")
     ap.add_argument("--leaf-order", type=int, default=0, choices=[0, 1], help="0 = ORB order (default), 1 = longest source list first")
     ap.add_argument("--maxleaf", type=int, default=0)

@@ -298,6 +298,7 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
             S.cur[st + (int)dst] = p[r];
             sub[r] = 2 * k + (el[r] - st >= (int)left);       // the sub-node of POSITION el[r] one level down
         }
+        if (level + 1 < depth)       // (the last level may have ORB_B_MAXSUB sub-nodes: nothing follows it)
         for (int k = threadIdx.x; k < nsub; k += blockDim.x) {
             const int st = sstart[k];
             sstart_next[2 * k] = st;

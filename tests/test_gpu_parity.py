@@ -233,7 +233,7 @@ def test_pairs_evaluated_and_list_cover(B, c1):
 
 
 @pytest.mark.parametrize("n,maxleaf,clustered", [(32768, 32, False), (20011, 16, False), (5000, 64, False), (262144, 32, True),
-                                                 (100003, 32, True)])
+                                                 (100003, 32, True), (262144, 16, True), (300007, 16, False)])
 def test_orb_tree_is_a_median_split_along_the_widest_axis(B, n, maxleaf, clustered):
     """PAPER.md L35 / DESIGN.md A13, checked on the device-built tree itself: every node is cut along the widest axis of
     its particle bounding box (fp32 coordinates), the left child takes floor(size/2) particles and no particle of the
