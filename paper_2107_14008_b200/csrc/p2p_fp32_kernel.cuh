@@ -385,10 +385,11 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
     // stage st of the ring: shared-memory addresses kept in registers, stage index and phase bit stepped by hand
     const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
     auto issue = [&](int k, int cur_batch, int st) {
-        const uint2 e = entry(k, cur_batch);
+        const uint2 mine = (k >> 5) == cur_batch ? dcur : dnext;       // warp-uniform choice; lane (k & 31) holds entry k
         if (MIXED) {
-            // origin differences in fp64, rounded once (A15); computed when the copy is issued, three runs
+            // origin differences in fp64, rounded once (A15); computed when the copy is issued, N_STAGES runs
             // ahead of their use, so the global loads of the origins are off the critical path
+            const uint2 e = make_uint2(__shfl_sync(0xffffffffu, mine.x, k & 31), __shfl_sync(0xffffffffu, mine.y, k & 31));
             const int nleaf = (int)((e.y & 0xffffu) >> a.log2m);
             if (lane < nleaf) {
                 const long long jl = (long long)(e.x >> a.log2m) + lane;
@@ -399,17 +400,21 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
             }
             __syncwarp();   // the stores above are read by other lanes (first N_STAGES entries: before any loop barrier)
         }
-        if (lane == 0) {
-            const uint32_t bytes = (e.y & 0xffffu) * 16u;
+        if (lane == (k & 31)) {      // the lane that holds the entry issues its copy: no shuffle on the producer side
+            const uint32_t bytes = (mine.y & 0xffffu) * 16u;
             mbar_expect_tx_u32(bars_u32 + 8u * st, bytes);
-            bulk_g2s_u32(ring_u32 + (uint32_t)(st * stage_bytes), a.p32 + (size_t)e.x * 4, bytes, bars_u32 + 8u * st);
+            bulk_g2s_u32(ring_u32 + (uint32_t)(st * stage_bytes), a.p32 + (size_t)mine.x * 4, bytes, bars_u32 + 8u * st);
         }
     };
     for (int k = 0; k < N_STAGES && k < n_my; ++k) issue(k, 0, k);
 
+    // stage and phase bit of entry k: with a power-of-two ring depth they are bit fields of k (no loop-carried state)
+    constexpr bool POW2_STAGES = (N_STAGES & (N_STAGES - 1)) == 0;
+    constexpr int LOG2_STAGES = N_STAGES == 2 ? 1 : N_STAGES == 4 ? 2 : N_STAGES == 8 ? 3 : 0;
     int st = 0;
     uint32_t phase = 0;
     for (int k = 0; k < n_my; ++k) {
+        if (POW2_STAGES) { st = k & (N_STAGES - 1); phase = (uint32_t)(k >> LOG2_STAGES) & 1u; }
         const int batch = k >> 5;
         if ((k & 31) == 0 && k > 0) { dcur = dnext; dnext = load_batch(batch + 1); }
         const uint2 e = entry(k, batch);
@@ -437,12 +442,17 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                 // L = Lh + Ll (two floats).  s = +1: move the target by -L: t - Lh is exact (it sits in the upper half
                 // of the box), then - Ll; s = -1: move the sources by -Lh per pair (exact for the same reason) and
                 // the target by +Ll.  With a box length that fp32 holds exactly Ll = 0.
-                sax = sxi < 0 ? -a.Lh : 0.f; say = syi < 0 ? -a.Lh : 0.f; saz = szi < 0 ? -a.Lh : 0.f;
+                if (((e.y >> 16) & 0x3fu) == 0x15u) {        // no image shift on any axis (most entries): warp-uniform
 #pragma unroll
-                for (int t = 0; t < T; ++t) {
-                    qx[t] = sxi > 0 ? (tx[t] - a.Lh) - a.Ll : sxi < 0 ? tx[t] + a.Ll : tx[t];
-                    qy[t] = syi > 0 ? (ty[t] - a.Lh) - a.Ll : syi < 0 ? ty[t] + a.Ll : ty[t];
-                    qz[t] = szi > 0 ? (tz[t] - a.Lh) - a.Ll : szi < 0 ? tz[t] + a.Ll : tz[t];
+                    for (int t = 0; t < T; ++t) { qx[t] = tx[t]; qy[t] = ty[t]; qz[t] = tz[t]; }
+                } else {
+                    sax = sxi < 0 ? -a.Lh : 0.f; say = syi < 0 ? -a.Lh : 0.f; saz = szi < 0 ? -a.Lh : 0.f;
+#pragma unroll
+                    for (int t = 0; t < T; ++t) {
+                        qx[t] = sxi > 0 ? (tx[t] - a.Lh) - a.Ll : sxi < 0 ? tx[t] + a.Ll : tx[t];
+                        qy[t] = syi > 0 ? (ty[t] - a.Lh) - a.Ll : syi < 0 ? ty[t] + a.Ll : ty[t];
+                        qz[t] = szi > 0 ? (tz[t] - a.Lh) - a.Ll : szi < 0 ? tz[t] + a.Ll : tz[t];
+                    }
                 }
             }
             const bool seam = (sax != 0.f) | (say != 0.f) | (saz != 0.f);
@@ -525,7 +535,8 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                 }
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    px[t] += pax[t].x + pax[t].y; py[t] += pay[t].x + pay[t].y; pz[t] += paz[t].x + paz[t].y;
+                    if (MIXED) { px[t] += pax[t].x + pax[t].y; py[t] += pay[t].x + pay[t].y; pz[t] += paz[t].x + paz[t].y; }
+                    else { px[t] = pax[t].x + pax[t].y; py[t] = pay[t].x + pay[t].y; pz[t] = paz[t].x + paz[t].y; }   // one block per run
                 }
             }
         }
@@ -555,7 +566,7 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
         for (int t = 0; t < T; ++t) { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
         __syncwarp();
         if (k + N_STAGES < n_my) issue(k + N_STAGES, batch, st);
-        if (++st == N_STAGES) { st = 0; phase ^= 1u; }
+        if (!POW2_STAGES) { if (++st == N_STAGES) { st = 0; phase ^= 1u; } }
     }
 
 #pragma unroll
