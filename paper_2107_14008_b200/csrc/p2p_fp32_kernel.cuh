@@ -434,8 +434,9 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
             // targets as seen from this block: d = (r_j + sadd) - q
             float qx[T], qy[T], qz[T];
             float sax = 0.f, say = 0.f, saz = 0.f;
+            float4 dc = make_float4(0.f, 0.f, 0.f, 0.f);
             if (MIXED) {
-                const float4 dc = cshift[st * MAX_RUN_LEAVES + (b0 >> a.log2m)];
+                dc = cshift[st * MAX_RUN_LEAVES + (b0 >> a.log2m)];
 #pragma unroll
                 for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dc.x; qy[t] = ty[t] - dc.y; qz[t] = tz[t] - dc.z; }
             } else {
@@ -460,18 +461,29 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
             const int np = blk / 2;
 
             if (per_pair) {
-                // degenerate geometry (tiny N, leaves spanning half the box): minimum image per pair
+                // degenerate geometry (tiny N, leaves spanning half the box): minimum image per pair.  The image shift is
+                // applied to an operand it is exact for, never to the rounded difference: ABS: x_j - x_i > L/2 puts x_j
+                // in the upper half of the box, so x_j - Lh is exact (and x_i - Lh when the sign is the other way);
+                // MIXED: to the origin difference.  A close pair across a box face then keeps its separation to one ulp
+                // of the separation, not of the box length.
+                auto image = [&](float xj, float xt, float dcx) {
+                    if (MIXED) {
+                        const float off = xj - xt;
+                        const float i = rintf((off + dcx) * a.invL);
+                        return off + fmaf(-a.Ll, i, fmaf(-a.Lh, i, dcx));
+                    }
+                    const float i = rintf((xj - xt) * a.invL);
+                    const float xs = i > 0.f ? xj - a.Lh : xj, ts = i < 0.f ? xt - a.Lh : xt;
+                    return fmaf(-a.Ll, i, xs - ts);
+                };
                 for (int p = half; p < np; p += pstep) {
                     const float4 A = s4[2 * p], B = s4[2 * p + 1];
 #pragma unroll
                     for (int t = 0; t < T; ++t) {
 #pragma unroll
                         for (int hh = 0; hh < 2; ++hh) {
-                            float dx = (hh ? A.y : A.x) - qx[t], dy = (hh ? A.w : A.z) - qy[t], dz = (hh ? B.y : B.x) - qz[t];
-                            const float ix = rintf(dx * a.invL), iy = rintf(dy * a.invL), iz = rintf(dz * a.invL);
-                            dx = fmaf(-a.Ll, ix, fmaf(-a.Lh, ix, dx));
-                            dy = fmaf(-a.Ll, iy, fmaf(-a.Lh, iy, dy));
-                            dz = fmaf(-a.Ll, iz, fmaf(-a.Lh, iz, dz));
+                            const float dx = image(hh ? A.y : A.x, tx[t], dc.x), dy = image(hh ? A.w : A.z, ty[t], dc.y),
+                                        dz = image(hh ? B.y : B.x, tz[t], dc.z);
                             float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.r2add)));
                             const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);

@@ -519,6 +519,20 @@ def test_softened_parity(B, oracle, c1, eps_over_rcut):
         assert _err(out[tgt], ref4) <= tol, (prec, g, kw)
 
 
+@pytest.mark.parametrize("precision,g_mode", [("fp32", "direct"), ("fp32", "poly"), ("mixed", "poly")])
+def test_per_pair_image_keeps_close_pairs_across_a_box_face(B, oracle, precision, g_mode):
+    """Tiny N (16^3, r_cut = 0.45 L): every list entry takes the minimum image per pair.  With softening the exact path
+    does not trigger, so the fp32 image arithmetic itself is on test: the shift must go to an operand it is exact for,
+    or a close pair across a box face loses its separation to one ulp of the box length (1.2e-5 rms before the fix)."""
+    cfg = workloads.scaled(1, 16)
+    pos, mass = workloads.make(cfg)
+    r_s, r_cut = _geom(cfg)
+    eps = 0.01 * r_cut
+    ref, _ = oracle.p2p(pos, mass, boxsize=cfg.boxsize, r_s=r_s, r_cut=r_cut, G=cfg.G, eps=eps)
+    out, st = _run(B, cfg, pos, mass, precision=precision, g_mode=g_mode, softening=eps, close_pair_radius=0.0)
+    assert _err(out, ref) <= 0.5 * TOL_FP32
+
+
 def test_softening_changes_the_answer_and_zero_is_bitwise_off(B, c1):
     cfg, pos, mass, ref, _ = c1
     r_s, r_cut = _geom(cfg)
