@@ -62,8 +62,8 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
         return {4: 56.0, 3: 51.0}.get(table_level, 51.0 - 4.0 * (3 - table_level))
     if g_mode == "poly":           # (8 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
         return 2.0 * (8 + poly_degree) + 3 + 2 + 1
-    if g_mode == "table":          # 512 nodes, level 2: 9 FFMA + 6 FADD + 10 FMUL + 1 MUFU
-        return 2.0 * 9 + 6 + 10 + 1 + 2.0 * (table_level - 2)
+    if g_mode == "table":          # level 2: 11 FFMA + 4 FADD + 8 FMUL + 1 MUFU = 35; one FFMA per level
+        return 2.0 * 11 + 4 + 8 + 1 + 2.0 * (table_level - 2)
     if g_mode == "fused":          # hand-fused erfc/exp: see profiles/r2_sass_inner_loop.md
         return FUSED_FLOPS_PER_PAIR
     # direct = stock erfcf + expf: 31 FFMA + 16 FMUL + 10 FADD + 5 MUFU (3 FFMA2 + 1.5 FADD2 packed among them)

@@ -50,7 +50,7 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     a.tn = c->table.n;
     a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
     a.uk = a.tn ? (float)(a.tn / 3.0 / (2.0 * rs)) : 0.f;
-    a.umax = (float)a.tn;
+    a.rmax = (float)(3.0 * 2.0 * rs);       // x = 3 = the last node
     a.table = c->table.d_TE;
     a.out = out; a.out_f32 = out_f32 ? 1 : 0;
 }

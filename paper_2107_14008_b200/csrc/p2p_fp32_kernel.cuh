@@ -65,7 +65,7 @@ struct P32Args {
     float tk;                  // POLY: t = r2 * tk - 1
     float ek, tmap;            // FUSED: exp(-x^2) = ex2(r2 * ek); t = x * tmap - 1 maps [0, x_cut] to [-1, 1]
     float pc[POLY_MAX_DEG + 1];
-    float uk, h, umax;         // TABLE: u = r * uk in node units, h = 3/n, umax = last node
+    float uk, h, rmax;         // TABLE: u = r * uk in node units, h = 3/n, rmax = radius of the last node
     int tn;
     const float2* table;
     void* out;
@@ -88,6 +88,13 @@ __device__ __forceinline__ float ex2(float x)
     return y;
 }
 __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+// 8-byte shared-memory load from a 32-bit shared address
+__device__ __forceinline__ float2 lds_f2(uint32_t addr)
+{
+    float2 v;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // g-dependent part of the pair core: returns w = G m_j g(r) / r^3 for two pairs at once.
@@ -130,15 +137,18 @@ template <int LEVEL>
 __device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* __restrict__ tab, float2 r2, float2 gm)
 {
     const float2 idr = f2(rsq(r2.x), rsq(r2.y));
-    // u = x n/3 in node units, clamped to the last node (FMNMX, ALU pipe) so that the index stays in range
-    float2 u = __fmul2_rn(__fmul2_rn(r2, idr), dup(a.uk));
-    u = f2(fminf(u.x, a.umax), fminf(u.y, a.umax));
-    const float2 um = __fadd2_rn(u, dup(MAGIC));             // nearest node (A14)
+    // r clamped to the last node's radius (FMNMX, ALU pipe) so that the index stays in range; the nearest node (A14) by
+    // the magic-number add folded into one FMA: u = r uk in node units, bits(u + 1.5 * 2^23) = bits(MAGIC) + node
+    float2 r = __fmul2_rn(r2, idr);
+    r = f2(fminf(r.x, a.rmax), fminf(r.y, a.rmax));
+    const float2 um = __ffma2_rn(r, dup(a.uk), dup(MAGIC));
     const float2 fi = __fadd2_rn(um, dup(-MAGIC));
-    const float2 eps = __fmul2_rn(__fadd2_rn(u, f2(-fi.x, -fi.y)), dup(a.h));
     const float2 xi = __fmul2_rn(fi, dup(a.h));
-    const float2 te0 = tab[__float_as_int(um.x) & 0x1fff];
-    const float2 te1 = tab[__float_as_int(um.y) & 0x1fff];
+    const float2 eps = __ffma2_rn(r, dup(a.inv2rs), f2(-xi.x, -xi.y));        // x - x_i, one rounding
+    // table address straight from the float's bit pattern: (bits << 3) + (base - (bits(MAGIC) << 3)), one LEA per lookup
+    const uint32_t tab_bias = smem_u32(tab) - (0x4B400000u << 3);
+    const float2 te0 = lds_f2(((uint32_t)__float_as_int(um.x) << 3) + tab_bias);
+    const float2 te1 = lds_f2(((uint32_t)__float_as_int(um.y) << 3) + tab_bias);
     const float2 Ti = f2(te0.x, te1.x), Ei = f2(te0.y, te1.y);
     float2 T = Ti;
     if (LEVEL >= 1) {
