@@ -70,7 +70,7 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
     return 2.0 * 31 + 16 + 10 + 5
 
 
-FUSED_FLOPS_PER_PAIR = 2.0 * (7 + 10) + 8 + 3 + 2   # degree 10: 17 FFMA + 8 FMUL + 3 FADD + MUFU.RSQ + MUFU.EX2
+FUSED_FLOPS_PER_PAIR = 2.0 * (7 + 10) + 7 + 3 + 2   # degree 10: 17 FFMA + 7 FMUL + 3 FADD + MUFU.RSQ + MUFU.EX2
 
 
 def peak_tflops(precision: str, sm_mhz: float) -> float:

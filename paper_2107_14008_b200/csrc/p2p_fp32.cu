@@ -46,7 +46,7 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
     a.tk = (float)(2.0 / (smax * 4.0 * rs * rs));
     for (int i = 0; i <= POLY_MAX_DEG; ++i) a.pc[i] = c->p.g_mode == PHOTONS_G_FUSED ? c->fused_c[i] : c->poly_c[i];
     a.ek = (float)(-1.4426950408889634 / (4.0 * rs * rs));          // exp(-x^2) = 2^(-x^2 log2 e), x^2 = r^2 / 4 r_s^2
-    a.tmap = (float)(2.0 / (0.5 * c->p.rcut_over_rs));
+    a.tmap = (float)(2.0 / (0.5 * c->p.rcut_over_rs) / (2.0 * rs));   // t = 2 x / x_cut - 1 with x = r / 2 r_s folded in
     a.tn = c->table.n;
     a.h = a.tn ? (float)(3.0 / a.tn) : 0.f;
     a.uk = a.tn ? (float)(a.tn / 3.0 / (2.0 * rs)) : 0.f;

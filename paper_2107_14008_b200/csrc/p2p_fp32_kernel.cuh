@@ -63,7 +63,7 @@ struct P32Args {
     double oscale, inv_oscale; // kernel-unit sums -> caller units: gmscale / pscale^2
     float inv2rs;              // 1 / 2 r_s (kernel units)
     float tk;                  // POLY: t = r2 * tk - 1
-    float ek, tmap;            // FUSED: exp(-x^2) = ex2(r2 * ek); t = x * tmap - 1 maps [0, x_cut] to [-1, 1]
+    float ek, tmap;            // FUSED: exp(-x^2) = ex2(r2 * ek); t = r * tmap - 1 maps r in [0, r_cut] to [-1, 1]
     float pc[POLY_MAX_DEG + 1];
     float uk, h, rmax;         // TABLE: u = r * uk in node units, h = 3/n, rmax = radius of the last node
     int tn;
@@ -122,8 +122,7 @@ template <int DEG>
 __device__ __forceinline__ float2 weight_fused(const P32Args& a, float2 r2, float2 gm)
 {
     const float2 idr = f2(rsq(r2.x), rsq(r2.y));
-    const float2 x = __fmul2_rn(__fmul2_rn(r2, idr), dup(a.inv2rs));
-    const float2 t = __ffma2_rn(x, dup(a.tmap), dup(-1.0f));
+    const float2 t = __ffma2_rn(__fmul2_rn(r2, idr), dup(a.tmap), dup(-1.0f));
     const float2 y = __fmul2_rn(r2, dup(a.ek));
     const float2 e = f2(ex2(y.x), ex2(y.y));
     float2 q = dup(a.pc[0]);
@@ -236,8 +235,7 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
             idr[c] = f2(rsq(r2[c].x), rsq(r2[c].y));
-            const float2 x = __fmul2_rn(__fmul2_rn(r2[c], idr[c]), dup(kc.inv2rs));
-            t[c] = __ffma2_rn(x, dup(kc.tmap), dup(-1.0f));
+            t[c] = __ffma2_rn(__fmul2_rn(r2[c], idr[c]), dup(kc.tmap), dup(-1.0f));
             const float2 y = __fmul2_rn(r2[c], dup(kc.ek));
             e[c] = f2(ex2(y.x), ex2(y.y));
             q[c] = __ffma2_rn(dup(kc.pc[0]), t[c], dup(kc.pc[1]));
