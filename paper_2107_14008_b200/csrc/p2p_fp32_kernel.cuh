@@ -438,6 +438,12 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
 #pragma unroll
         for (int t = 0; t < T; ++t) px[t] = py[t] = pz[t] = 0.f;
 
+        // the same, packed (the two sources of a pair accumulate side by side).  MIXED: one set for all the blocks
+        // (source leaves) of the run; ABS: one block per run, declared where it is used (shorter live ranges)
+        float2 pax_run[T], pay_run[T], paz_run[T];
+#pragma unroll
+        for (int t = 0; t < T; ++t) pax_run[t] = pay_run[t] = paz_run[t] = dup(0.f);
+
         for (int b0 = 0; b0 < ns; b0 += blk) {
             // targets as seen from this block: d = (r_j + sadd) - q
             float qx[T], qy[T], qz[T];
@@ -499,12 +505,15 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                     }
                 }
             } else {
-                float2 nqx[T], nqy[T], nqz[T], pax[T], pay[T], paz[T];
+                float2 nqx[T], nqy[T], nqz[T], pax_blk[T], pay_blk[T], paz_blk[T];
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     nqx[t] = dup(-qx[t]); nqy[t] = dup(-qy[t]); nqz[t] = dup(-qz[t]);
-                    pax[t] = pay[t] = paz[t] = dup(0.f);
+                    pax_blk[t] = pay_blk[t] = paz_blk[t] = dup(0.f);
                 }
+                float2 (&pax)[T] = MIXED ? pax_run : pax_blk;
+                float2 (&pay)[T] = MIXED ? pay_run : pay_blk;
+                float2 (&paz)[T] = MIXED ? paz_run : paz_blk;
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
                 // U source pairs x T targets = NCH independent chains per iteration
                 // (with lane groups the leaf's np = maxleaf/2 source pairs are shared out, so fewer fit in one iteration)
@@ -553,11 +562,16 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                 } else {
                     for (int p = half; p < np; p += pstep * U) step(p, false);
                 }
+                if (!MIXED) {
 #pragma unroll
-                for (int t = 0; t < T; ++t) {
-                    if (MIXED) { px[t] += pax[t].x + pax[t].y; py[t] += pay[t].x + pay[t].y; pz[t] += paz[t].x + paz[t].y; }
-                    else { px[t] = pax[t].x + pax[t].y; py[t] = pay[t].x + pay[t].y; pz[t] = paz[t].x + paz[t].y; }   // one block per run
+                    for (int t = 0; t < T; ++t) { px[t] = pax[t].x + pax[t].y; py[t] = pay[t].x + pay[t].y; pz[t] = paz[t].x + paz[t].y; }
                 }
+            }
+        }
+        if (MIXED) {     // (px is non-zero only after the per-pair path, which does not use the packed sums)
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                px[t] += pax_run[t].x + pax_run[t].y; py[t] += pay_run[t].x + pay_run[t].y; pz[t] += paz_run[t].x + paz_run[t].y;
             }
         }
         // Exact path: a run whose partial sum is larger than one pair at close_pair_radius would give holds a pair
