@@ -409,6 +409,7 @@ struct ListArgs {
     long long* n_chunks_of;       // pass 1: per leaf
     unsigned long long* totals;   // pass 1: [0] leaf pairs, [1] pairs evaluated, [2] longest list in source slots
     long long* work_of;           // pass 1: slots in the list of each leaf (for the heaviest-first order)
+    int4* resume;                 // per leaf: walk state when the stash filled up {heap index, run_first, run_n, run_code}
 };
 
 __global__ void list_kernel(ListArgs a)
@@ -427,23 +428,33 @@ __global__ void list_kernel(ListArgs a)
 
     int run_first = -1, run_n = 0, run_code = -1, n_chunks = 0, n_pairs = 0;
     long long n_eval = 0;
-    // Pass 1 counts and keeps the first stash_cap entries of every leaf; pass 2 (only the leaves whose list
-    // did not fit, the rest is a plain copy by list_copy_kernel) walks again and writes in place.
-    const bool skip = !live || (a.chunks && a.n_chunks_of[i] <= a.stash_cap);
-    uint2* out = a.chunks ? a.chunks + a.chunk_ptr[i] : nullptr;
-    uint2* stash = a.chunks ? nullptr : a.stash + i * a.stash_cap;
+    // Pass 1 counts and keeps the first stash_cap entries of every leaf, and notes the state of the walk at the moment
+    // the stash fills up; pass 2 (only the leaves whose list did not fit; the stashed part is copied by
+    // list_copy_kernel) resumes the walk from that state and writes the rest in place.
+    const bool pass2 = a.chunks != nullptr;
+    const bool skip = !live || (pass2 && a.n_chunks_of[i] <= a.stash_cap);
+    uint2* out = pass2 ? a.chunks + a.chunk_ptr[i] : nullptr;
+    uint2* stash = pass2 ? nullptr : a.stash + i * a.stash_cap;
     const int max_leaves_per_chunk = a.chunk_max / a.maxleaf;
+    unsigned h = skip ? 0u : 1u;
     auto emit = [&]() {
         const uint2 ent = make_uint2((unsigned)(run_first * a.maxleaf), (unsigned)(run_n * a.maxleaf) | (unsigned)run_code);
         if (out) out[n_chunks] = ent;
         else if (n_chunks < a.stash_cap) stash[n_chunks] = ent;
         ++n_chunks;
     };
+    if (pass2 && !skip) {      // continue after the leaf that opened run number stash_cap
+        const int4 r = a.resume[i];
+        h = (unsigned)r.x; run_first = r.y; run_n = r.z; run_code = r.w;
+        n_chunks = a.stash_cap;
+        const unsigned up = h + 1;
+        h = up >> (__ffs(up) - 1);
+        if (h == 1) h = 0;
+    }
 
     // Stackless depth-first walk of the complete binary tree: with 1-based heap indices the children of h are 2h and
     // 2h + 1, and the node that follows the subtree of h is (h + 1) >> ctz(h + 1) (up while h is a right child, then
     // on to the sibling); arriving at 1 = back at the root = done.  Left child first: leaves come out in ascending order.
-    unsigned h = skip ? 0u : 1u;
     while (h) {
         const int node = (int)h - 1;
         const float4 nc = __ldg(&a.box[2 * (size_t)node]), nhw = __ldg(&a.box[2 * (size_t)node + 1]);
@@ -470,7 +481,10 @@ __global__ void list_kernel(ListArgs a)
             if (run_n > 0 && j == run_first + run_n && code == run_code && run_n < max_leaves_per_chunk) {
                 ++run_n;
             } else {
-                if (run_n > 0) emit();
+                if (run_n > 0) {
+                    emit();
+                    if (!pass2 && n_chunks == a.stash_cap) a.resume[i] = make_int4((int)h, j, 1, code);   // state after this leaf
+                }
                 run_first = j; run_n = 1; run_code = code;
             }
         }
@@ -512,15 +526,14 @@ __global__ void node_box32_kernel(long long n_nodes, const double* __restrict__ 
     box[2 * k + 1] = make_float4(h[0], h[1], h[2], 0.f);
 }
 
-// one warp per leaf: stash -> CSR for the lists that fitted into the stash
+// one warp per leaf: stash -> CSR
 __global__ void list_copy_kernel(long long n_leaves, int stash_cap, const long long* __restrict__ chunk_ptr,
                                  const uint2* __restrict__ stash, uint2* __restrict__ chunks)
 {
     const long long i = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     if (i >= n_leaves) return;
     const long long c0 = chunk_ptr[i];
-    const int cnt = (int)(chunk_ptr[i + 1] - c0);
-    if (cnt > stash_cap) return;
+    const int cnt = min((int)(chunk_ptr[i + 1] - c0), stash_cap);     // longer lists: list_kernel's second pass writes the rest
     for (int k = threadIdx.x & 31; k < cnt; k += 32) chunks[c0 + k] = stash[i * stash_cap + k];
 }
 
@@ -703,6 +716,7 @@ int build_leaves_impl(Ctx* c)
     la.chunk_ptr = nullptr; la.chunks = nullptr; la.n_chunks_of = d_nch; la.totals = d_tot; la.work_of = d_work;
     la.stash_cap = LIST_STASH;
     PH_WS(la.stash, uint2, WS_LIST_STASH, n_leaves * LIST_STASH);
+    PH_WS(la.resume, int4, WS_LIST_RESUME, n_leaves);
     list_kernel<<<blocks_for(n_leaves, 64), 64, 0, st>>>(la);
     ++c->launches;
     {

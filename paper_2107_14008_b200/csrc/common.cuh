@@ -50,7 +50,7 @@ enum WsSlot {
     WS_PERM, WS_ORB_P0, WS_ORB_P1, WS_ORB_KEYS, WS_ORB_KEYS2, WS_ORB_VALS, WS_ORB_VALS2, WS_ORB_LO, WS_ORB_HI, WS_CUB_TMP,
     WS_LEAF_CNT, WS_NODE_LO, WS_NODE_HI, WS_NODE_BOX32, WS_LEAF_CTR, WS_SLOT_SRC, WS_P64, WS_P32,
     WS_SEL_NODE, WS_SEL_CNT, WS_SEL_Q0, WS_SEL_C0, WS_SEL_HIST, WS_SEL_NODEVAR, WS_SEL_CNT2, WS_SEL_BASE2, WS_SEL_LO2, WS_SEL_HI2,
-    WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_LIST_STASH, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
+    WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_LIST_STASH, WS_LIST_RESUME, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
     WS_COUNT
 };
 struct DevBuf { void* p = nullptr; size_t cap = 0; };

@@ -272,6 +272,29 @@ def test_orb_tree_is_a_median_split_along_the_widest_axis(B, n, maxleaf, cluster
                 assert left.max() <= right.min() + ext[axis] * 2.0 ** -20, (level, k, axis)
 
 
+def test_long_lists_take_the_second_walk_and_agree(B, c1):
+    """Lists longer than the builder's stash (128 entries) are finished by a second walk that resumes where the first
+    one ran out of stash.  With runs of a single leaf (chunk_max = maxleaf = 16) every list of config 1 is that long;
+    the set of (target leaf, source leaf, image) triples must equal the one built with runs of 8 leaves."""
+    cfg, pos, mass, _, _ = c1
+    got = []
+    for chunk_max in (16, 128):
+        with B.Photons(n_pm=cfg.n_pm, maxleaf=16, chunk_max=chunk_max, precision="fp64", g_mode="direct") as ph:
+            ph.set_particles(pos, mass)
+            ph.build_leaves()
+            st = ph.stats()
+            ptr, first, nleaf, code = ph.interaction_list()
+        tl = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+        trip = np.concatenate([np.stack([np.full(k, t), np.arange(f, f + k), np.full(k, c)], axis=1)
+                               for t, f, k, c in zip(tl, first, nleaf, code)])
+        got.append((st, np.diff(ptr), trip[np.lexsort(trip.T[::-1])]))
+    (st_a, len_a, trip_a), (st_b, len_b, trip_b) = got
+    assert len_a.min() > 128 and len_b.max() <= 128          # the first build needed the second walk everywhere
+    assert (nleaf_ok := st_a["n_leaf_pairs"]) == st_b["n_leaf_pairs"] == len(trip_a) == len(trip_b)
+    assert np.array_equal(trip_a, trip_b)
+    assert st_a["pairs_evaluated"] == st_b["pairs_evaluated"]
+
+
 # ------------------------------------------------------------------- ragged sizes and degenerate cases
 
 @pytest.mark.parametrize("n", [1, 2, 3, 31, 33, 100, 1000, 5000, 20011])
