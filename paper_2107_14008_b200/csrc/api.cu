@@ -361,8 +361,8 @@ int photons_short_range_acc(photons_ctx* ctx, void* acc, int dtype, int mem_kind
     }
 
     // target-leaf batches round-robin over the streams (north_star: "stream concurrency between leaf
-    // batches"; "concurrency management").  The order array is heaviest-first, so batch b
-    // takes every n_streams-th block of it.
+    // batches"; "concurrency management"): the order array (photons_params.leaf_order) is cut into
+    // 4 n_streams contiguous blocks, block b goes to stream b mod n_streams.
     const int ns = (int)c->streams.size();
     const long long nl = c->n_leaves;
     const long long n_batches = ns == 1 ? 1 : (long long)ns * 4;
