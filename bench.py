@@ -58,6 +58,8 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
             return 129.0           # the static count is 180, warp votes skip erfc/exp where no lane is inside the cut
         if table_layout == "coef":  # level 4: 15 DFMA + 7 DMUL + 4 DADD + 1 MUFU; one DFMA per level
             return 2.0 * (11 + table_level) + 7 + 4 + 1
+        if table_layout == "quad":  # level 4: 16 DFMA + 10 DMUL + 4 DADD + 1 MUFU (the brackets of T[3], T[4] are read)
+            return 2.0 * (12 + table_level) + 10 + 4 + 1
         # paper layout: level 4: 20 DFMA + 11 DMUL + 4 DADD + 1 MUFU; level 3: 18 + 10 + 4 + 1
         return {4: 56.0, 3: 51.0}.get(table_level, 51.0 - 4.0 * (3 - table_level))
     if g_mode == "poly":           # (8 + d) FFMA + 3 FADD + 2 FMUL + 1 MUFU.RSQ
@@ -614,7 +616,7 @@ def main(argv=None):
     ap.add_argument("--g-mode", dest="g_mode", default="poly", choices=["poly", "table", "direct", "fused"])
     ap.add_argument("--table-nodes", type=int, default=512)
     ap.add_argument("--table-level", type=int, default=2)
-    ap.add_argument("--table-layout", default="paper", choices=["paper", "coef"])
+    ap.add_argument("--table-layout", default="paper", choices=["paper", "coef", "quad"])
     ap.add_argument("--softening-over-rcut", type=float, default=0.0)
     ap.add_argument("--warps-per-leaf", type=int, default=0)
     ap.add_argument("--chunk-max", type=int, default=0, help="longest staged run in source slots (0 = the library default)")

@@ -67,8 +67,10 @@ enum {
 /* what the interpolation table holds per node (PHOTONS_G_TABLE) */
 enum {
     PHOTONS_TABLE_PAPER = 0, /* {T_i, E_i} as in the paper (L143); the polynomials of Eq. 2 in x_i are rebuilt per pair */
-    PHOTONS_TABLE_COEF = 1   /* the Taylor coefficients of Eq. 2 themselves, T^(k)(x_i) h^k / k!, k = 0..table_level: the
+    PHOTONS_TABLE_COEF = 1,  /* the Taylor coefficients of Eq. 2 themselves, T^(k)(x_i) h^k / k!, k = 0..table_level: the
                                 same series about the same node, Horner only (PHOTONS_FP64 only) */
+    PHOTONS_TABLE_QUAD = 2   /* {T_i, E_i} plus the two highest node polynomials of Eq. 2, the brackets of T[3] and T[4]
+                                (L137-L141), tabulated instead of rebuilt per pair: 32 bytes per node (PHOTONS_FP64 only) */
 };
 
 enum { PHOTONS_MEM_HOST = 0, PHOTONS_MEM_DEVICE = 1 };
@@ -110,7 +112,7 @@ typedef struct {
     double softening;         /* Plummer softening length eps >= 0 (A23): the pair function is
                                  taken at r_eps = sqrt(r^2 + eps^2), a_i += G m_j d_ij g(r_eps) / r_eps^3 for pairs with
                                  0 < r and r_eps < r_cut.  0 = none (default; north_star's formula) */
-    int table_layout;         /* TABLE: PHOTONS_TABLE_PAPER (default) or PHOTONS_TABLE_COEF */
+    int table_layout;         /* TABLE: PHOTONS_TABLE_PAPER (default), PHOTONS_TABLE_COEF or PHOTONS_TABLE_QUAD */
     int leaf_order;           /* order in which CTAs take the target leaves: 0 = ORB order (default: neighbouring leaves run
                                  together and share their source leaves in L2), 1 = longest source list first */
     int orb_method;           /* upper levels of the ORB build: 0 = radix-select partition of every node about its median

@@ -23,7 +23,8 @@ DTYPE_F64, DTYPE_F32 = 0, 1
 
 PRECISIONS = {"fp64": FP64, "fp32": FP32, "mixed": MIXED}
 G_MODES = {"direct": G_DIRECT, "table": G_TABLE, "poly": G_POLY, "fused": G_FUSED}
-TABLE_LAYOUTS = {"paper": TABLE_PAPER, "coef": TABLE_COEF}
+TABLE_QUAD = 2
+TABLE_LAYOUTS = {"paper": TABLE_PAPER, "coef": TABLE_COEF, "quad": TABLE_QUAD}
 ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX", "ENONFINITE"]
 
 EXPORTS = [

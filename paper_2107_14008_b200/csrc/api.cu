@@ -170,10 +170,10 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
         if (p.table_level < 0 || p.table_level > 4) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_level must be 0..4");
         if (p.table_level > 3 && p.precision != PHOTONS_FP64)
             return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_level 4 needs PHOTONS_FP64 (the fp32 kernels keep T[0..3])");
-        if (p.table_layout != PHOTONS_TABLE_PAPER && p.table_layout != PHOTONS_TABLE_COEF)
+        if (p.table_layout != PHOTONS_TABLE_PAPER && p.table_layout != PHOTONS_TABLE_COEF && p.table_layout != PHOTONS_TABLE_QUAD)
             return create_fail(err_buf, err_len, PHOTONS_EINVAL, "bad table_layout");
-        if (p.table_layout == PHOTONS_TABLE_COEF && p.precision != PHOTONS_FP64)
-            return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF is an option of the PHOTONS_FP64 path");
+        if (p.table_layout != PHOTONS_TABLE_PAPER && p.precision != PHOTONS_FP64)
+            return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF / QUAD are options of the PHOTONS_FP64 path");
     }
     if (p.orb_method != 0 && p.orb_method != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "orb_method must be 0 or 1");
     if (p.leaf_order != 0 && p.leaf_order != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "leaf_order must be 0 or 1");
@@ -465,6 +465,7 @@ void photons_destroy(photons_ctx* ctx)
     cudaFree(c->table.d_TE);
     cudaFree(c->table.d_TE64);
     cudaFree(c->table.d_C64);
+    cudaFree(c->table.d_Q64);
     if (!c->streams.empty()) c->streams[0] = c->own_stream0;
     for (auto s : c->streams) if (s) cudaStreamDestroy(s);
     for (auto e : c->stream_done) if (e) cudaEventDestroy(e);

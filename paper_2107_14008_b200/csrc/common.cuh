@@ -39,6 +39,7 @@ struct GTable {                 // Eq. 2 table
     float2* d_TE = nullptr;     // {T_i, E_i} per node (fp32)
     double2* d_TE64 = nullptr;  // fp64 copy for the fp64 path
     double* d_C64 = nullptr;    // coefficient layout (PHOTONS_TABLE_COEF): 5 doubles per node, T^(k)(x_i) h^k / k!
+    double* d_Q64 = nullptr;    // PHOTONS_TABLE_QUAD: {T_i, E_i, bracket of T[3], bracket of T[4]} per node
 };
 
 constexpr int POLY_MAX_DEG = 20;

@@ -19,7 +19,7 @@ int make_table(Ctx* c)
     const int n = c->p.table_nodes;
     std::vector<float2> te(n + 1);
     std::vector<double2> te64(n + 1);
-    std::vector<double> c64((size_t)(n + 1) * 5);
+    std::vector<double> c64((size_t)(n + 1) * 5), q64((size_t)(n + 1) * 4);
     const long double h = 3.0L / n;
     for (int i = 0; i <= n; ++i) {
         const long double x = 3.0L * i / n;                                  // nodes over x in [0, 3] (L143)
@@ -33,6 +33,10 @@ int make_table(Ctx* c)
                                    -x * (x2 * x2 / 3.0L - 1.5L * x2 + 1.0L) * E};
         long double hk = 1.0L;
         for (int k = 0; k < 5; ++k) { c64[(size_t)i * 5 + k] = (double)(ck[k] * hk); hk *= h; }
+        // quad layout: the paper's pair and the brackets of T[3] and T[4] (polynomials in x_i, L137-L141)
+        q64[(size_t)i * 4] = (double)T; q64[(size_t)i * 4 + 1] = (double)E;
+        q64[(size_t)i * 4 + 2] = (double)(2.0L / 3.0L * x2 * x2 - 5.0L / 3.0L * x2 + 1.0L / 3.0L);
+        q64[(size_t)i * 4 + 3] = (double)(-x * (x2 * x2 / 3.0L - 1.5L * x2 + 1.0L));
     }
     c->table.n = n;
     c->table.level = c->p.table_level;
@@ -42,6 +46,8 @@ int make_table(Ctx* c)
     PH_CUDA(c, cudaMemcpy(c->table.d_TE64, te64.data(), sizeof(double2) * (n + 1), cudaMemcpyHostToDevice));
     PH_CUDA(c, cudaMalloc(&c->table.d_C64, sizeof(double) * c64.size()));
     PH_CUDA(c, cudaMemcpy(c->table.d_C64, c64.data(), sizeof(double) * c64.size(), cudaMemcpyHostToDevice));
+    PH_CUDA(c, cudaMalloc(&c->table.d_Q64, sizeof(double) * q64.size()));
+    PH_CUDA(c, cudaMemcpy(c->table.d_Q64, q64.data(), sizeof(double) * q64.size(), cudaMemcpyHostToDevice));
     return PHOTONS_OK;
 }
 

@@ -30,7 +30,7 @@ constexpr double MAGIC64 = 6755399441055744.0;   // 1.5 * 2^52
 constexpr int N_STAGES64 = 2;
 constexpr int TAB_STRIDE = 5;             // doubles per node in the coefficient layout (odd: fewer bank conflicts)
 
-enum { G64_DIRECT = 0, G64_TABLE = 1, G64_COEF = 2 };
+enum { G64_DIRECT = 0, G64_TABLE = 1, G64_COEF = 2, G64_QUAD = 3 };
 
 struct P64Args {
     const double4* p64;       // n_slots x {x, y, z, G m}
@@ -92,6 +92,22 @@ __device__ __forceinline__ void g_eval(const P64Args& a, const double* __restric
 #pragma unroll
             for (int k = LEVEL - 1; k >= 0; --k) p = fma(p, eu, t[k]);
             g[c] = p;
+        }
+    } else if (GMODE == G64_QUAD) {
+        // Eq. 2 with the brackets of T[3] and T[4] read from the table beside {T_i, E_i}: 9 DP instructions instead of 14
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const double2 te = reinterpret_cast<const double2*>(tab)[2 * idx[c]];
+            const double2 hi = reinterpret_cast<const double2*>(tab)[2 * idx[c] + 1];
+            const double xi = fi[c] * a.h;
+            const double e = fma(r[c], a.inv2rs, -xi);
+            const double xi2 = xi * xi;
+            double poly = 0.0;
+            if (LEVEL >= 4) poly = hi.y;
+            if (LEVEL >= 3) poly = fma(poly, e, hi.x);
+            if (LEVEL >= 2) poly = fma(poly, e, fma(-xi, xi2, xi));
+            if (LEVEL >= 1) poly = fma(poly, e, xi2);
+            g[c] = LEVEL >= 1 ? fma(te.y * e, poly, te.x) : te.x;
         }
     } else {
         // Eq. 2 to level LEVEL about the nearest node, the node polynomials rebuilt from x_i
@@ -308,6 +324,7 @@ static int launch_g(Ctx* c, const P64Args& a, long long count, int W, size_t sme
 {
     if (c->p.g_mode == PHOTONS_G_DIRECT) return launch_t<T, LG, G64_DIRECT, 0>(c, a, count, W, smem, st);
     if (c->p.table_layout == PHOTONS_TABLE_COEF) return launch_l<T, LG, G64_COEF>(c, a, count, W, smem, st);
+    if (c->p.table_layout == PHOTONS_TABLE_QUAD) return launch_l<T, LG, G64_QUAD>(c, a, count, W, smem, st);
     return launch_l<T, LG, G64_TABLE>(c, a, count, W, smem, st);
 }
 
@@ -320,12 +337,12 @@ int launch_p2p_fp64(Ctx* c, long long first, long long count, void* out, bool ou
     // start value of the r^2 chain: eps^2 (A23), else a floor far below any separation, scaled with r_cut^2 so that
     // it means the same in any units
     a.r2add = c->p.softening > 0 ? c->p.softening * c->p.softening : R2_FLOOR64 * a.rcut2;
-    const bool coef = c->p.table_layout == PHOTONS_TABLE_COEF;
+    const bool coef = c->p.table_layout == PHOTONS_TABLE_COEF, quad = c->p.table_layout == PHOTONS_TABLE_QUAD;
     a.table = nullptr; a.tn = 0; a.tab_doubles = 0;
     if (c->p.g_mode == PHOTONS_G_TABLE) {
         a.tn = c->table.n;
-        a.table = coef ? c->table.d_C64 : reinterpret_cast<const double*>(c->table.d_TE64);
-        a.tab_doubles = (a.tn + 1) * (coef ? TAB_STRIDE : 2);
+        a.table = coef ? c->table.d_C64 : quad ? c->table.d_Q64 : reinterpret_cast<const double*>(c->table.d_TE64);
+        a.tab_doubles = (a.tn + 1) * (coef ? TAB_STRIDE : quad ? 4 : 2);
         a.h = 3.0 / a.tn;
         a.uk = a.tn / 3.0 * a.inv2rs;
     }

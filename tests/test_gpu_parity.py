@@ -574,9 +574,11 @@ def test_softening_changes_the_answer_and_zero_is_bitwise_off(B, c1):
 @pytest.mark.parametrize("maxleaf", [16, 32, 64, 128])
 @pytest.mark.parametrize("layout,nodes,level,tol", [("paper", 512, 4, 1e-10), ("coef", 512, 4, 1e-10), ("paper", 4096, 3, TOL_FP64),
                                                    ("coef", 4096, 3, TOL_FP64), ("coef", 4096, 4, TOL_FP64),
-                                                   ("coef", 256, 2, TOL_TABLE), ("paper", 256, 1, TOL_TABLE), ("coef", 1024, 0, 1e-3)])
+                                                   ("coef", 256, 2, TOL_TABLE), ("paper", 256, 1, TOL_TABLE), ("coef", 1024, 0, 1e-3),
+                                                   ("quad", 512, 4, 1e-10), ("quad", 4096, 3, TOL_FP64), ("quad", 256, 2, TOL_TABLE),
+                                                   ("quad", 256, 0, 1e-2)])
 def test_c1_fp64_table_layouts(B, c1, maxleaf, layout, nodes, level, tol):
-    # Eq. 2 in fp64, both table layouts: the same Taylor series about the same node.  512 nodes / T[4]
+    # Eq. 2 in fp64, all three table layouts: the same Taylor series about the same node.  512 nodes / T[4]
     # ("T[4] for double") carries the table's own truncation error, ~5e-12 in T (SURVEY §8(c) "table")
     cfg, pos, mass, ref, _ = c1
     out, _ = _run(B, cfg, pos, mass, precision="fp64", g_mode="table", table_nodes=nodes, table_level=level,
