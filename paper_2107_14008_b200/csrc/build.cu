@@ -33,7 +33,10 @@ void free_leaves(Ctx* c)
 // Splitting coordinates are the positions rounded to fp32; ties go either way, which never changes `a`.
 
 constexpr int ORB_CTA_MAX = 4096;   // particles a phase-B CTA holds in shared memory
-constexpr int ORB_CTA_THREADS = 1024;
+#ifndef PHOTONS_ORB_CTA_THREADS
+#define PHOTONS_ORB_CTA_THREADS 1024
+#endif
+constexpr int ORB_CTA_THREADS = PHOTONS_ORB_CTA_THREADS;
 // Phase-A sort key = (node, coordinate quantised to this many bits inside the node's bbox).  20 bits resolve 1e-6 of
 // the node's extent — far below the particle spacing of nodes that still hold > 4096 particles — and keep the
 // keys within 32 bits (4 radix passes or fewer) down to level 12; ties are split by the stable order.
@@ -145,7 +148,7 @@ struct OrbBShared {
     unsigned wtot[ORB_B_WARPS], wbase[ORB_B_WARPS];
 };
 
-__global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, int L0, int depth, const float4* __restrict__ P,
+__global__ void __launch_bounds__(ORB_CTA_THREADS, ORB_CTA_THREADS >= 1024 ? 1 : 2) orb_cta_kernel(long long n, int L0, int depth, const float4* __restrict__ P,
                                                                   uint32_t* __restrict__ perm)
 {
     extern __shared__ __align__(16) unsigned char orb_smem[];
@@ -264,14 +267,14 @@ __global__ void __launch_bounds__(ORB_CTA_THREADS) orb_cta_kernel(long long n, i
         }
         __syncthreads();
         if (warp == 0) {
-            const unsigned v = S.wtot[lane];
+            const unsigned v = lane < ORB_B_WARPS ? S.wtot[lane] : 0u;
             unsigned inc = v;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
                 if (lane >= o) inc += t;
             }
-            S.wbase[lane] = inc - v;
+            if (lane < ORB_B_WARPS) S.wbase[lane] = inc - v;
         }
         __syncthreads();
 #pragma unroll

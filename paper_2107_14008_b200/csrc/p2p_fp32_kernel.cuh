@@ -517,7 +517,7 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                 const float2 sx2 = dup(sax), sy2 = dup(say), sz2 = dup(saz);
                 // U source pairs x T targets = NCH independent chains per iteration
                 // (with lane groups the leaf's np = maxleaf/2 source pairs are shared out, so fewer fit in one iteration)
-                constexpr int U = T == 1 ? (HS == 1 ? PHOTONS_UNROLL_T1 : PHOTONS_UNROLL_T1 / 2) : T == 2 ? (HS == 4 ? 2 : PHOTONS_UNROLL_T2) : 1;
+                constexpr int U = T == 1 ? (HS == 1 ? PHOTONS_UNROLL_T1 : (PHOTONS_UNROLL_T1 / 2 > 4 ? 4 : PHOTONS_UNROLL_T1 / 2)) : T == 2 ? (HS == 4 ? 2 : PHOTONS_UNROLL_T2) : 1;
                 static_assert(U * HS <= 16 * T / HS, "a leaf's source pairs must fill whole iterations");
                 constexpr int NCH = U * T;
                 auto step = [&](const int p, const bool with_seam) {
