@@ -439,6 +439,7 @@ def run_sweep(args):
     variants += [("mixed", "direct", {}), ("mixed", "poly", {}), ("mixed", "table", dict(table_nodes=512, table_level=2))]
     variants += [("fp64", "direct", {}), ("fp64", "table", dict(table_nodes=512, table_level=4)),
                  ("fp64", "table", dict(table_nodes=512, table_level=4, table_layout="coef")),
+                 ("fp64", "table", dict(table_nodes=512, table_level=4, table_layout="quad")),
                  ("fp64", "table", dict(table_nodes=4096, table_level=3)),
                  ("fp64", "table", dict(table_nodes=4096, table_level=3, table_layout="coef"))]
     peak32 = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9
@@ -461,7 +462,7 @@ def run_sweep(args):
             err = float(np.sqrt(((a - ref) ** 2).sum(axis=1)).max() / rms)
             ms = min(ks)
             rate = st["pairs_evaluated"] / (ms * 1e-3)
-            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]" + (" coef" if extra.get("table_layout") == "coef" else "")
+            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]" + (" " + extra["table_layout"] if extra.get("table_layout") else "")
             print(f"| {maxleaf} | {prec} | {gname} | {st['pairs_evaluated']:.4g} | {ms:.2f} | {rate:.3e} | "
                   f"{in_cut_per_particle * cfg.n / (ms * 1e-3):.3e} | {rate * PAPER_FLOPS_PER_PAIR / 1e12:.1f} | "
                   f"{100 * rate * PAPER_FLOPS_PER_PAIR / peak32:.1f} | {err:.2e} |", flush=True)
