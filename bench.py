@@ -434,6 +434,7 @@ def run_sweep(args):
     out = torch.empty((cfg.n, 3), dtype=torch.float64, device="cuda")
     close = CLOSE_OVER_RCUT[cfg.kind] * r_cut
     variants = [("fp32", "direct", {}), ("fp32", "fused", {}), ("fp32", "poly", {})]
+    variants += [("fp32", "poly", dict(poly_degree=d)) for d in (10, 11, 13)]      # the default is 12
     variants += [("fp32", "table", dict(table_nodes=n, table_level=2)) for n in (256, 512, 1024, 4096)]
     variants += [("fp32", "table", dict(table_nodes=512, table_level=lv)) for lv in (0, 1, 3)]
     variants += [("mixed", "direct", {}), ("mixed", "poly", {}), ("mixed", "table", dict(table_nodes=512, table_level=2))]
@@ -452,6 +453,8 @@ def run_sweep(args):
         for prec, g, extra in variants:
             if args.sweep_quick and (maxleaf != 32 and (g == "table" and extra.get("table_nodes") != 512 or extra.get("table_level", 2) != 2)):
                 continue
+            if "poly_degree" in extra and maxleaf != 32:
+                continue
             params = headline_params(cfg, maxleaf=maxleaf, precision=prec, g_mode=g, close_pair_radius=close if prec != "fp64" else 0.0, **extra)
             with B.Photons(**params) as ph:
                 ph.set_particles(d_pos, None)
@@ -462,7 +465,7 @@ def run_sweep(args):
             err = float(np.sqrt(((a - ref) ** 2).sum(axis=1)).max() / rms)
             ms = min(ks)
             rate = st["pairs_evaluated"] / (ms * 1e-3)
-            gname = g if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]" + (" " + extra["table_layout"] if extra.get("table_layout") else "")
+            gname = (g + (f" degree {extra['poly_degree']}" if "poly_degree" in extra else "")) if g != "table" else f"table {extra['table_nodes']} / T[{extra['table_level']}]" + (" " + extra["table_layout"] if extra.get("table_layout") else "")
             print(f"| {maxleaf} | {prec} | {gname} | {st['pairs_evaluated']:.4g} | {ms:.2f} | {rate:.3e} | "
                   f"{in_cut_per_particle * cfg.n / (ms * 1e-3):.3e} | {rate * PAPER_FLOPS_PER_PAIR / 1e12:.1f} | "
                   f"{100 * rate * PAPER_FLOPS_PER_PAIR / peak32:.1f} | {err:.2e} |", flush=True)
