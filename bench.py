@@ -49,10 +49,13 @@ PAPER_FLOPS_PER_PAIR = 51.0
 
 
 def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGREE, table_level: int = 2,
-                   table_layout: str = "paper") -> float:
+                   table_layout: str = "paper", equal_mass: bool = False) -> float:
     """Executed flops per evaluated pair, counted in the SASS of each kernel's hot loop (profiles/r2_sass_inner_loop.md;
     ncu's op_ffma counters read 0 for the packed FFMA2 stream): FFMA/DFMA = 2, FADD/FMUL/DADD/DMUL = 1, MUFU = 1,
-    compares and selects 0."""
+    compares and selects 0.  equal_mass: the fp32 POLY / TABLE / FUSED kernels that the library takes when all masses
+    are equal (photons_params.mass_path = 0) leave the multiply by G m_j out of the pair core: one FMUL per pair less."""
+    if equal_mass and precision == "fp32" and g_mode in ("poly", "table", "fused"):
+        return flops_per_pair(precision, g_mode, poly_degree=poly_degree, table_level=table_level, table_layout=table_layout) - 1.0
     if precision == "fp64":
         if g_mode == "direct":     # executed per pair on config 4 (ncu DFMA/DMUL/DADD counters): 52.6 + 12.7 + 7.8 + 3 MUFU;
             return 129.0           # the static count is 180, warp votes skip erfc/exp where no lane is inside the cut
@@ -287,6 +290,8 @@ def run_ours(args):
         params["chunk_max"] = args.chunk_max
     if args.leaf_order:
         params["leaf_order"] = args.leaf_order
+    if args.mass_path:
+        params["mass_path"] = args.mass_path
     if args.no_close or args.precision == "fp64":
         params["close_pair_radius"] = 0.0
     n = cfg.n
@@ -350,7 +355,9 @@ def run_ours(args):
     line = None
     if rank == 0:
         kernel_ms = float(np.mean(k_ms))
-        fpp = flops_per_pair(args.precision, args.g_mode, table_level=args.table_level, table_layout=args.table_layout)
+        # (the synthetic workloads have one particle species: mass = NULL = 1/n each)
+        fpp = flops_per_pair(args.precision, args.g_mode, table_level=args.table_level, table_layout=args.table_layout,
+                             equal_mass=not args.mass_path)
         clocks = clk.summary()
         peak_tf = peak_tflops(args.precision, clocks["sm_max_mhz"] or 1965.0)
         achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
@@ -388,6 +395,8 @@ def run_ours(args):
             "config": {"workload": cfg0.name, "n_particles": n, "n_pm": cfg.n_pm, "maxleaf": params["maxleaf"],
                        "precision": args.precision, "g_mode": args.g_mode, "close_pair_radius_over_rcut": params["close_pair_radius"] / r_cut,
                        "n_streams": args.streams, "input_flavour": "F (fp32-grid positions)",
+                       "masses": "equal (one particle species, mass = NULL); " + ("G m_j per pair forced (mass_path 1)" if args.mass_path or args.precision != "fp32" or args.g_mode == "direct"
+                                                                                   else "equal-mass kernels: G m applied once per staged run (mass_path 0)"),
                        "l2": "inputs exceed L2 (leaf-sorted particles + interaction list > 126 MB); no flush",
                        "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "step": "set_particles + build_leaves + short_range_acc"},
@@ -626,6 +635,8 @@ def main(argv=None):
     ap.add_argument("--chunk-max", type=int, default=0, help="longest staged run in source slots (0 = the library default)")
     ap.add_argument("--targets-per-lane", type=int, default=0, help="register tiling of the fp32 kernels (0 = the default of the leaf size)")
     ap.add_argument("--leaf-order", type=int, default=0, choices=[0, 1], help="0 = ORB order (default), 1 = longest source list first")
+    ap.add_argument("--mass-path", type=int, default=0, choices=[0, 1],
+                    help="0 = equal masses take the kernels that apply G m once per run (default), 1 = always G m_j per pair")
     ap.add_argument("--maxleaf", type=int, default=0)
     ap.add_argument("--streams", type=int, default=1)
     ap.add_argument("--no-close", action="store_true", help="switch the exact close-pair path off")

@@ -43,6 +43,7 @@ class Params(ctypes.Structure):
         ("close_pair_radius", ctypes.c_double), ("chunk_max", ctypes.c_int), ("warps_per_leaf", ctypes.c_int),
         ("targets_per_lane", ctypes.c_int), ("poly_degree", ctypes.c_int), ("periodic", ctypes.c_int),
         ("softening", ctypes.c_double), ("table_layout", ctypes.c_int), ("leaf_order", ctypes.c_int), ("orb_method", ctypes.c_int),
+        ("mass_path", ctypes.c_int),
     ]
 
 

@@ -63,7 +63,9 @@ static double now_ms()
 }
 
 // wrap into [0, L), flag non-finite values, find max |m| (the fp32 kernels' mass unit); src is fp64 or fp32.
-// flags: [0] = non-finite input seen, [1] = bits of max |m| (non-negative doubles order like their bit patterns)
+// flags: [0] = non-finite input seen, [1] = bits of max |m| (non-negative doubles order like their bit patterns),
+// [2] = bits of min |m| (starts at all ones), [3] = signs seen (1 = negative, 2 = positive): all masses are equal iff
+// [1] == [2] and only one sign was seen
 template <typename Tin>
 __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Tin* __restrict__ mass, double L, int periodic,
                               double default_mass, double* __restrict__ opos, double* __restrict__ omass,
@@ -90,6 +92,10 @@ __global__ void intake_kernel(long long n, const Tin* __restrict__ pos, const Ti
     unsigned long long mb = (unsigned long long)__double_as_longlong(fabs(m));
     for (int o = 16; o > 0; o >>= 1) mb = max(mb, __shfl_xor_sync(0xffffffffu, mb, o));
     if ((threadIdx.x & 31) == 0 && mb > 0) atomicMax(&flags[1], mb);
+    unsigned long long mn = (unsigned long long)__double_as_longlong(fabs(m));
+    unsigned sg = m < 0.0 ? 1u : m > 0.0 ? 2u : 0u;
+    for (int o = 16; o > 0; o >>= 1) { mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o)); sg |= __shfl_xor_sync(0xffffffffu, sg, o); }
+    if ((threadIdx.x & 31) == 0) { atomicMin(&flags[2], mn); if (sg) atomicOr(&flags[3], (unsigned long long)sg); }
 }
 
 // build_ms from the events recorded around photons_build_leaves' device work
@@ -141,6 +147,7 @@ void photons_default_params(photons_params* p)
     p->table_layout = PHOTONS_TABLE_PAPER;
     p->leaf_order = 0;
     p->orb_method = 0;
+    p->mass_path = 0;
 }
 
 static int create_fail(char* err_buf, int err_len, int code, const char* msg)
@@ -176,6 +183,7 @@ int photons_create(const photons_params* pp, photons_ctx** out, char* err_buf, i
             return create_fail(err_buf, err_len, PHOTONS_EINVAL, "table_layout COEF / QUAD are options of the PHOTONS_FP64 path");
     }
     if (p.orb_method != 0 && p.orb_method != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "orb_method must be 0 or 1");
+    if (p.mass_path != 0 && p.mass_path != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "mass_path must be 0 or 1");
     if (p.leaf_order != 0 && p.leaf_order != 1) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "leaf_order must be 0 or 1");
     if (p.n_streams < 1 || p.n_streams > 64) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "n_streams must be 1..64");
     if (p.close_pair_radius < 0 || !std::isfinite(p.close_pair_radius)) return create_fail(err_buf, err_len, PHOTONS_EINVAL, "close_pair_radius must be >= 0");
@@ -277,7 +285,7 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     const size_t esz = dtype == PHOTONS_DTYPE_F64 ? 8 : 4;
     c->d_pos = static_cast<double*>(workspace(c, WS_POS, sizeof(double) * 3 * n));
     c->d_mass = static_cast<double*>(workspace(c, WS_MASS, sizeof(double) * n));
-    unsigned long long* d_flags = static_cast<unsigned long long*>(workspace(c, WS_FLAG, 2 * sizeof(unsigned long long)));
+    unsigned long long* d_flags = static_cast<unsigned long long*>(workspace(c, WS_FLAG, 4 * sizeof(unsigned long long)));
     if (!c->d_pos || !c->d_mass || !d_flags) { free_particles(c); return PHOTONS_ENOMEM; }
     const void *src_pos = pos, *src_mass = mass;
     if (mem_kind == PHOTONS_MEM_HOST) {
@@ -292,7 +300,8 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
             src_mass = d_in_mass;
         }
     }
-    PH_CUDA(c, cudaMemsetAsync(d_flags, 0, 2 * sizeof(unsigned long long), st));
+    PH_CUDA(c, cudaMemsetAsync(d_flags, 0, 4 * sizeof(unsigned long long), st));
+    PH_CUDA(c, cudaMemsetAsync(d_flags + 2, 0xff, sizeof(unsigned long long), st));
     const int tb = 256;
     const unsigned nb = (unsigned)((n + tb - 1) / tb);
     if (dtype == PHOTONS_DTYPE_F64)
@@ -300,7 +309,7 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     else
         intake_kernel<float><<<nb, tb, 0, st>>>(n, (const float*)src_pos, (const float*)src_mass, c->p.boxsize, c->p.periodic, 1.0 / (double)n, c->d_pos, c->d_mass, d_flags);
     ++c->launches;
-    unsigned long long h_flags[2] = {0, 0};
+    unsigned long long h_flags[4] = {0, 0, 0, 0};
     cudaError_t e = cudaMemcpyAsync(h_flags, d_flags, sizeof h_flags, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { free_particles(c); return fail(c, PHOTONS_ECUDA, "set_particles: %s", cudaGetErrorString(e)); }
@@ -311,6 +320,11 @@ int photons_set_particles(photons_ctx* ctx, long long n, const void* pos, const 
     const double gm_max = std::fabs(c->p.G) * m_max;
     c->gm_max = gm_max;
     c->gmscale = gm_max > 0 && std::isfinite(gm_max) ? std::ldexp(1.0, (int)std::ceil(std::log2(gm_max))) : 1.0;
+    // all masses equal (the paper's runs: one particle species; Alg. 2 L177 carries a single GM): the fp32 kernels then
+    // apply G m once per staged run instead of once per pair
+    c->gm_uniform = 0.0;
+    if (m_max > 0 && h_flags[1] == h_flags[2] && (h_flags[3] == 1 || h_flags[3] == 2))
+        c->gm_uniform = c->p.G * (h_flags[3] == 1 ? -m_max : m_max);
     c->n = n;
     return PHOTONS_OK;
 }

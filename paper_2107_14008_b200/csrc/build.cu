@@ -346,8 +346,9 @@ __global__ void leaf_table_kernel(long long n, int depth, long long n_leaves, co
 }
 
 // one thread per slot: fill the packed arrays.  Padding slots repeat the leaf's first particle with
-// zero mass (they add nothing as sources and are never written as targets).
-__global__ void pack_kernel(long long n, int depth, int maxleaf, long long n_slots, double G, int precision,
+// zero mass (they add nothing as sources and are never written as targets).  ugm (equal-mass fp32 kernels, which do
+// not read G m per pair): the fp32 copy of a padding slot sits far outside the box instead, beyond r_cut of everything.
+__global__ void pack_kernel(long long n, int depth, int maxleaf, long long n_slots, double G, int precision, int ugm,
                             double inv_pscale, double inv_gmscale,
                             const uint32_t* __restrict__ perm, const double* __restrict__ pos,
                             const double* __restrict__ mass, const double* __restrict__ ctr,
@@ -371,9 +372,10 @@ __global__ void pack_kernel(long long n, int depth, int maxleaf, long long n_slo
         if (precision == PHOTONS_MIXED) { ox = ctr[3 * k]; oy = ctr[3 * k + 1]; oz = ctr[3 * k + 2]; }
         float* b = p32 + (s >> 1) * 8 + (s & 1);
         // kernel units (powers of two: the rescaling itself is exact)
-        b[0] = (float)((x - ox) * inv_pscale);
-        b[2] = (float)((y - oy) * inv_pscale);
-        b[4] = (float)((z - oz) * inv_pscale);
+        const bool away = ugm && !real;
+        b[0] = away ? PAD_FAR : (float)((x - ox) * inv_pscale);
+        b[2] = away ? PAD_FAR : (float)((y - oy) * inv_pscale);
+        b[4] = away ? PAD_FAR : (float)((z - oz) * inv_pscale);
         b[6] = (float)(gm * inv_gmscale);
     }
 }
@@ -686,7 +688,9 @@ int build_leaves_impl(Ctx* c)
         double* leaf_lo = c->d_node_lo + 3 * (n_leaves - 1);
         double* leaf_hi = c->d_node_hi + 3 * (n_leaves - 1);
         leaf_table_kernel<<<blocks_for(n_leaves, 128), 128, 0, st>>>(n, depth, n_leaves, c->d_perm, c->d_pos, c->d_leaf_cnt, leaf_lo, leaf_hi, c->d_leaf_ctr);
-        pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, 1.0 / c->pscale, 1.0 / c->gmscale,
+        // equal masses (set_particles) and a kernel that can leave G m out of the pair core (photons_params.mass_path)
+        c->ugm = c->gm_uniform != 0.0 && c->p.mass_path == 0 && c->p.precision == PHOTONS_FP32 && c->p.g_mode != PHOTONS_G_DIRECT;
+        pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, c->ugm ? 1 : 0, 1.0 / c->pscale, 1.0 / c->gmscale,
                                                             c->d_perm, c->d_pos, c->d_mass,
                                                             c->d_leaf_ctr, c->d_slot_src, c->d_p64, c->d_p32);
         c->launches += 2;

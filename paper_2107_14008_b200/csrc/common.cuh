@@ -54,6 +54,9 @@ enum WsSlot {
     WS_LIST_NCH, WS_LIST_WORK, WS_LIST_TOT, WS_LIST_STASH, WS_LIST_RESUME, WS_CHUNK_PTR, WS_CHUNKS, WS_ORDER, WS_ORDER_KEYS, WS_ORDER_KEYS2, WS_ORDER_VALS,
     WS_COUNT
 };
+// fp32 coordinate (kernel units, r_cut in [1, 2)) of a padding slot in the equal-mass kernels: r^2 ~ 3e30 stays finite
+constexpr float PAD_FAR = 1.0e15f;
+
 struct DevBuf { void* p = nullptr; size_t cap = 0; };
 
 struct Ctx {
@@ -64,6 +67,8 @@ struct Ctx {
     // in fp64 by gmscale / pscale^2 when they are stored
     double pscale = 1.0, gmscale = 1.0;
     double gm_max = 0.0;                 // max |G m_j| of the current particle set
+    double gm_uniform = 0.0;             // G m if every particle has the same mass, else 0
+    bool ugm = false;                    // the current leaves were packed for the equal-mass fp32 kernels (build_leaves)
     int sm_count = 0;
     std::vector<const void*> smem_opted;  // kernels whose dynamic shared-memory limit has been raised already
     std::vector<cudaStream_t> streams;   // [0] = main stream (the caller's after photons_set_stream)

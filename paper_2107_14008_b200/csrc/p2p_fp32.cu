@@ -41,6 +41,11 @@ void fill_p32_args(Ctx* c, P32Args& a, long long first, void* out, bool out_f32)
         const double pth = (c->gm_max / c->gmscale) / (rc * rc);
         a.pth2 = (float)std::fmin(pth * pth, 1e37);
     }
+    a.gmu = 1.0;
+    if (c->ugm) {      // the runs' fp32 partial sums lack the common factor G m: it is applied when they are flushed
+        a.gmu = c->gm_uniform / c->gmscale;
+        a.pth2 = (float)std::fmin((double)a.pth2 / (a.gmu * a.gmu), 1e37);
+    }
     a.inv2rs = (float)(1.0 / (2.0 * rs));
     const double smax = 0.25 * c->p.rcut_over_rs * c->p.rcut_over_rs;
     a.tk = (float)(2.0 / (smax * 4.0 * rs * rs));

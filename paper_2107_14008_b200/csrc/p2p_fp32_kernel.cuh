@@ -58,6 +58,7 @@ struct P32Args {
     float rcut2;               // kernel units; compared with r^2 + r2add
     float pth2;                // exact path: square of the run-partial acceleration that triggers it (kernel units); 0 = off
     float r2add;               // max(R2_FLOOR, eps^2): start value of every r^2 chain
+    double gmu;                // UGM kernels (all G m equal): the common G m in kernel units, applied once per run
     double Ld, inv2rs_d, rcut2_d, eps2_d;   // caller units, for the exact path
     double inv_pscale;         // 1 / Ctx::pscale
     double oscale, inv_oscale; // kernel-unit sums -> caller units: gmscale / pscale^2
@@ -132,7 +133,7 @@ __device__ __forceinline__ float2 weight_fused(const P32Args& a, float2 r2, floa
     return __fmul2_rn(__fmul2_rn(q, e), __fmul2_rn(idr2, __fmul2_rn(idr, gm)));
 }
 
-template <int LEVEL>
+template <int LEVEL, bool UGM>
 __device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* __restrict__ tab, float2 r2, float2 gm)
 {
     const float2 idr = f2(rsq(r2.x), rsq(r2.y));
@@ -167,7 +168,7 @@ __device__ __forceinline__ float2 weight_table(const P32Args& a, const float2* _
     }
     const float2 idr2 = __fmul2_rn(idr, idr);
     const float2 idr3 = __fmul2_rn(idr2, idr);
-    return __fmul2_rn(__fmul2_rn(idr3, T), gm);
+    return UGM ? __fmul2_rn(idr3, T) : __fmul2_rn(__fmul2_rn(idr3, T), gm);
 }
 
 // Eq. 1 by the CUDA library special functions (what the paper's §3.3 L121 calls expensive)
@@ -181,12 +182,12 @@ __device__ __forceinline__ float weight_direct1(const P32Args& a, float r2, floa
 
 enum { GM_POLY = 0, GM_TABLE = 1, GM_DIRECT = 2, GM_FUSED = 3 };
 
-template <int GKIND, int GPAR>
+template <int GKIND, int GPAR, bool UGM = false>
 __device__ __forceinline__ float2 weight2(const P32Args& a, const float2* tab, float2 r2, float2 gm)
 {
     float2 w;
     if (GKIND == GM_POLY) w = weight_poly<GPAR>(a, r2, gm);
-    else if (GKIND == GM_TABLE) w = weight_table<GPAR>(a, tab, r2, gm);
+    else if (GKIND == GM_TABLE) w = weight_table<GPAR, UGM>(a, tab, r2, gm);
     else if (GKIND == GM_FUSED) w = weight_fused<GPAR>(a, r2, gm);
     else w = f2(weight_direct1(a, r2.x, gm.x), weight_direct1(a, r2.y, gm.y));
     // the cut (A8) and, with it, everything the approximations do outside their range
@@ -203,7 +204,7 @@ struct LoopConst {
 };
 
 // SEL = false: the cut is left to the caller (acc_cut below), w is the raw value
-template <int GKIND, int GPAR, int NCH, bool SEL>
+template <int GKIND, int GPAR, int NCH, bool SEL, bool UGM>
 __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, const float2* tab, const float2 (&r2)[NCH],
                                         const float2 (&gm)[NCH], float2 (&w)[NCH])
 {
@@ -224,7 +225,7 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
         for (int c = 0; c < NCH; ++c) {
             const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
             const float2 u = __ffma2_rn(idr2, idr[c], f2(-q[c].x, -q[c].y));
-            const float2 v = __fmul2_rn(u, gm[c]);
+            const float2 v = UGM ? u : __fmul2_rn(u, gm[c]);
             w[c] = SEL ? f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f) : v;
         }
     } else if (GKIND == GM_FUSED) {
@@ -248,12 +249,12 @@ __device__ __forceinline__ void weights(const P32Args& a, const LoopConst& kc, c
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
             const float2 idr2 = __fmul2_rn(idr[c], idr[c]);
-            const float2 v = __fmul2_rn(__fmul2_rn(q[c], e[c]), __fmul2_rn(idr2, __fmul2_rn(idr[c], gm[c])));
+            const float2 v = __fmul2_rn(__fmul2_rn(q[c], e[c]), __fmul2_rn(idr2, UGM ? idr[c] : __fmul2_rn(idr[c], gm[c])));
             w[c] = SEL ? f2(r2[c].x < kc.rcut2 ? v.x : 0.f, r2[c].y < kc.rcut2 ? v.y : 0.f) : v;
         }
     } else {
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR>(a, tab, r2[c], gm[c]);    // (selects inside)
+        for (int c = 0; c < NCH; ++c) w[c] = weight2<GKIND, GPAR, UGM>(a, tab, r2[c], gm[c]);    // (selects inside)
     }
 }
 
@@ -313,7 +314,7 @@ static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64
 
 // ---------------------------------------------------------------------------------------------------------
 
-template <int T, int HS, bool MIXED, int GKIND, int GPAR>
+template <int T, int HS, bool MIXED, int GKIND, int GPAR, bool UGM = false>
 __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T2 : 1) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -499,7 +500,7 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                             const float dx = image(hh ? A.y : A.x, tx[t], dc.x), dy = image(hh ? A.w : A.z, ty[t], dc.y),
                                         dz = image(hh ? B.y : B.x, tz[t], dc.z);
                             float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.r2add)));
-                            const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(hh ? B.w : B.z));
+                            const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(UGM ? 1.f : hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
                         }
                     }
@@ -524,7 +525,14 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                     float2 dx[NCH], dy[NCH], dz[NCH], r2[NCH], gm[NCH], w[NCH];
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
-                        const float4 A = s4[2 * (p + u * pstep)], B = s4[2 * (p + u * pstep) + 1];
+                        const float4 A = s4[2 * (p + u * pstep)];
+                        float4 B;
+                        if (UGM) {   // all G m equal: only {z0, z1} of the second half is read (one LDS.64)
+                            const float2 Bz = *reinterpret_cast<const float2*>(&s4[2 * (p + u * pstep) + 1]);
+                            B = make_float4(Bz.x, Bz.y, 0.f, 0.f);
+                        } else {
+                            B = s4[2 * (p + u * pstep) + 1];
+                        }
                         float2 xj = f2(A.x, A.y), yj = f2(A.z, A.w), zj = f2(B.x, B.y);
                         if (with_seam) { xj = __fadd2_rn(xj, sx2); yj = __fadd2_rn(yj, sy2); zj = __fadd2_rn(zj, sz2); }
 #pragma unroll
@@ -539,7 +547,7 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                         r2[c] = __ffma2_rn(dx[c], dx[c], __ffma2_rn(dy[c], dy[c], __ffma2_rn(dz[c], dz[c], dup(kc.r2add))));
                     }
                     constexpr bool PRED = PHOTONS_PRED_ACC && T == 2 && HS == 1 && (GKIND == GM_POLY || GKIND == GM_FUSED);
-                    weights<GKIND, GPAR, NCH, !PRED>(a, kc, tab, r2, gm, w);
+                    weights<GKIND, GPAR, NCH, !PRED, UGM>(a, kc, tab, r2, gm, w);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
 #pragma unroll
@@ -597,7 +605,10 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
         }
         // level 2 of the accumulation: flush the run's fp32 partial sums into the fp64 sums
 #pragma unroll
-        for (int t = 0; t < T; ++t) { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
+        for (int t = 0; t < T; ++t) {
+            if (UGM) { ax[t] = fma((double)px[t], a.gmu, ax[t]); ay[t] = fma((double)py[t], a.gmu, ay[t]); az[t] = fma((double)pz[t], a.gmu, az[t]); }
+            else { ax[t] += (double)px[t]; ay[t] += (double)py[t]; az[t] += (double)pz[t]; }
+        }
         __syncwarp();
         if (k + N_STAGES < n_my) issue(k + N_STAGES, batch, st);
         if (!POW2_STAGES) { if (++st == N_STAGES) { st = 0; phase ^= 1u; } }
@@ -658,7 +669,10 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     const size_t smem = p32_smem_bytes(c, T);
     void (*kern)(P32Args) = nullptr;
     const bool mixed = c->p.precision == PHOTONS_MIXED;
-#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR> : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR>)
+    const bool ugm = c->ugm;     // equal masses: G m out of the pair core (never MIXED or DIRECT: build_leaves)
+    constexpr bool HAS_UGM = GKIND != GM_DIRECT;
+#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR> : ugm ? p2p_fp32_kernel<TT, HH, false, GKIND, GPAR, HAS_UGM> \
+                                : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR>)
     switch (M * 8 + T) {   // (MAXLEAF, targets per lane) -> (T, lane groups)
         case 16 * 8 + 1: kern = PH_SHAPE(1, 2); break;
         case 16 * 8 + 2: kern = PH_SHAPE(2, 4); break;

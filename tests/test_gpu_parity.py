@@ -382,6 +382,65 @@ def test_isolated_boundaries(B, oracle):
     assert _err(out, ref8) <= TOL_FP64
 
 
+@pytest.mark.parametrize("n,maxleaf", [(40, 32), (33, 16), (1000, 32), (5000, 64), (20011, 16), (20011, 32), (20011, 128)])
+@pytest.mark.parametrize("g_mode,tol", [("poly", TOL_FP32), ("fused", TOL_FP32), ("table", TOL_TABLE)])
+def test_equal_mass_kernels(B, oracle, n, maxleaf, g_mode, tol):
+    """photons_params.mass_path: with every mass equal (Alg. 2 L177 carries one GM) the fp32 kernels leave G m out of the
+    pair core and apply it once per staged run.  Ragged N, so that padding slots (which these kernels cannot silence by a
+    zero mass) are in every leaf; a G m that is not a power of two; against the oracle and against the per-pair path."""
+    rng = np.random.default_rng(500 + n)
+    pos = rng.random((n, 3)).astype(np.float32).astype(np.float64)
+    m0, G = 7.5 / n, 43.0
+    mass = np.full(n, m0)
+    n_pm = 16
+    r_s = 1.2 / n_pm
+    ref, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=6 * r_s, G=G)
+    kw = dict(n_pm=n_pm, G=G, precision="fp32", g_mode=g_mode, maxleaf=maxleaf, close_pair_radius=0.02 * 6 * r_s)
+    eq, st = B.short_range_acc(pos, mass, **kw)
+    per, _ = B.short_range_acc(pos, mass, mass_path=1, **kw)
+    none, _ = B.short_range_acc(pos * 1.0, None, **{**kw, "G": G * m0 * n})       # mass = NULL is 1/n each
+    assert _err(eq, ref) <= tol and _err(per, ref) <= tol and _err(none, ref) <= tol
+    assert _err(eq, per) <= 0.5 * TOL_FP32                             # two kernels, the same sum up to fp32 rounding
+    assert n < 1000 or not np.array_equal(eq, per)
+    # one particle of another mass: set_particles must notice and take the per-pair kernels
+    mass2 = mass.copy()
+    mass2[n // 2] *= 3.0
+    ref2, _ = oracle.p2p(pos, mass2, boxsize=1.0, r_s=r_s, r_cut=6 * r_s, G=G)
+    out2, _ = B.short_range_acc(pos, mass2, **kw)
+    assert _err(out2, ref2) <= tol
+
+
+def test_equal_mass_kernels_softened_isolated_and_negative(B, oracle):
+    rng = np.random.default_rng(91)
+    n, n_pm = 6001, 16
+    r_s = 1.2 / n_pm
+    r_cut = 6 * r_s
+    pos = rng.random((n, 3)).astype(np.float32).astype(np.float64)
+    mass = np.full(n, 1.0 / n)
+    kw = dict(n_pm=n_pm, precision="fp32", g_mode="poly", close_pair_radius=0.02 * r_cut)
+    ref, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=r_cut, eps=0.01 * r_cut)
+    out, _ = B.short_range_acc(pos, mass, softening=0.01 * r_cut, **kw)
+    assert _err(out, ref) <= TOL_FP32
+    # isolated boundaries: a blob that straddles the origin (as test_isolated_boundaries, with one mass)
+    blob = (rng.normal(0.0, 0.35, (n, 3)) + np.array([0.1, 0.9, -0.2])).astype(np.float32).astype(np.float64)
+    ref, _ = oracle.p2p(blob, mass, boxsize=0.0, r_s=1.2 / 32, r_cut=6 * 1.2 / 32)
+    out, _ = B.short_range_acc(blob, mass, periodic=0, **{**kw, "n_pm": 32, "close_pair_radius": 0.02 * 6 * 1.2 / 32})
+    assert _err(out, ref) <= TOL_FP32
+    ref, _ = oracle.p2p(pos, -mass, boxsize=1.0, r_s=r_s, r_cut=r_cut)          # equal negative masses: the sign is kept
+    out, _ = B.short_range_acc(pos, -mass, **kw)
+    assert _err(out, ref) <= TOL_FP32
+
+
+@pytest.mark.parametrize("maxleaf,tpl", [(16, 1), (16, 2), (32, 1), (32, 2), (64, 2), (128, 4)])
+def test_c1_per_pair_mass_path(B, c1, maxleaf, tpl):
+    # config 1 has equal masses, so every other config-1 test runs the equal-mass kernels: the per-pair ones here
+    cfg, pos, mass, ref, _ = c1
+    for g, tol in (("poly", TOL_FP32), ("fused", TOL_FP32), ("table", TOL_TABLE)):
+        out, _ = _run(B, cfg, pos, mass, precision="fp32", g_mode=g, maxleaf=maxleaf, targets_per_lane=tpl, mass_path=1,
+                      close_pair_radius=_close(cfg))
+        assert _err(out, ref) <= tol
+
+
 # ---------------------------------------------------------------------------- error behaviour (ABI)
 
 def test_abi_errors(B):
@@ -391,7 +450,7 @@ def test_abi_errors(B):
     assert e.value.code == B.EBOX
     for bad in (dict(maxleaf=48), dict(precision=7), dict(g_mode=9), dict(n_streams=0), dict(boxsize=-1.0),
                 dict(precision="fp64", g_mode="poly"), dict(g_mode="table", table_nodes=5),
-                dict(g_mode="poly", rcut_over_rs=7.0)):
+                dict(g_mode="poly", rcut_over_rs=7.0), dict(mass_path=2)):
         with pytest.raises(B.PhotonsError) as e:
             B.Photons(**bad)
         assert e.value.code == B.EINVAL
@@ -706,6 +765,7 @@ def test_full_size_config4_golden_10k(B):
             (bench.headline_params(cfg, g_mode="fused"), TOL_FP32),
             (bench.headline_params(cfg, g_mode="table", table_nodes=512, table_level=2), TOL_TABLE),
             (bench.headline_params(cfg, precision="mixed"), TOL_FP32), (bench.headline_params(cfg, maxleaf=16), TOL_FP32),
+            (bench.headline_params(cfg, mass_path=1), TOL_FP32),       # G m_j per pair (the equal-mass kernels are the default here)
             (bench.headline_params(cfg, precision="fp64", g_mode="table", table_nodes=4096, table_level=3), TOL_FP64)]
     for i, (params, tol) in enumerate(runs):
         with B.Photons(**params) as ph:
