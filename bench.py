@@ -362,6 +362,8 @@ def run_ours(args):
         peak_tf = peak_tflops(args.precision, clocks["sm_max_mhz"] or 1965.0)
         achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
         traffic, traffic_src = ncu_traffic(cfg0.name, params["maxleaf"], args.precision, args.g_mode)
+        if args.mass_path and args.precision == "fp32" and args.g_mode != "direct":
+            traffic, traffic_src = None, None      # the rows of these variants are captures of the equal-mass kernels
         f64 = args.precision == "fp64"
         roofline = {
             "bound": "alu", "kernel": "p2p_fp64_kernel" if f64 else "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf,
