@@ -226,6 +226,27 @@ int photons_m2l(int device, int p, double r_s, double boxsize, long long n_cells
                 const double* multipoles, const long long* pair_ptr, const int* pair_src, const signed char* pair_shift,
                 double* locals, int mem_kind, void* cuda_stream, double* kernel_ms);
 
+/* photons_m2l for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same operator, arguments and coefficient order as photons_m2l (A24-A26), with
+ * DEVICE pointers only (all of them on `device`; pair_shift may be NULL, pair_src may not), and a kernel variant that
+ * splits every target cell's source list over several warps and adds their partial L_n in a fixed order - the same sums
+ * as photons_m2l up to fp64 rounding order, reproducible from call to call.
+ * The partial sums live in a file-scope device array of PHOTONS_M2L_NOALLOC_SCRATCH_BYTES that every GPU which loads the
+ * library holds until the process exits.  The call enqueues two kernels on cuda_stream (a cudaStream_t, NULL = default
+ * stream) and returns WITHOUT synchronising; it calls no cudaMalloc / cudaFree / allocating library routine, creates no
+ * event or stream, and copies nothing.  (The first call on a device looks the array's device address up with
+ * cudaGetSymbolAddress: make one call outside any graph capture.)
+ * Limit: n_cells * NC(p) * 8 bytes <= PHOTONS_M2L_NOALLOC_SCRATCH_BYTES (29 959 cells at p = 4, 1 048 576 at p = 0);
+ * beyond it the call returns PHOTONS_EINVAL, launches nothing and says so in err_buf - use photons_m2l there.
+ * All calls on a device share the array: calls that can overlap on the GPU (different streams, different host threads)
+ * race on it - serialise them on one stream.  Nothing in it has to be cleared between calls.
+ * err_buf (may be NULL): err_len bytes for the message of a failing call.
+ * Errors: EINVAL (arguments, the limit), ENODEVICE, ECUDA. */
+#define PHOTONS_M2L_NOALLOC_SCRATCH_BYTES (8u << 20)
+int photons_m2l_noalloc(int device, int p, double r_s, double boxsize, long long n_cells, const double* centres,
+                        const double* multipoles, const long long* pair_ptr, const int* pair_src,
+                        const signed char* pair_shift, double* locals, void* cuda_stream, char* err_buf, int err_len);
+
 /* Message of the last failing call on ctx; valid until the next call on ctx. */
 const char* photons_last_error(const photons_ctx* ctx);
 

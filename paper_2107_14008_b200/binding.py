@@ -30,7 +30,7 @@ ERROR_NAMES = ["OK", "EINVAL", "ESTATE", "ENOMEM", "ECUDA", "ENODEVICE", "EBOX",
 EXPORTS = [
     "photons_default_params", "photons_create", "photons_set_stream", "photons_set_particles", "photons_build_leaves",
     "photons_short_range_acc", "photons_get_leaf_order", "photons_get_interaction_list", "photons_get_stats",
-    "photons_peak_probe", "photons_poly_fit", "photons_fused_fit", "photons_m2l", "photons_last_error", "photons_destroy",
+    "photons_peak_probe", "photons_poly_fit", "photons_fused_fit", "photons_m2l", "photons_m2l_noalloc", "photons_last_error", "photons_destroy",
 ]
 
 
@@ -105,6 +105,8 @@ def load():
     lib.photons_m2l.restype = ci
     lib.photons_m2l.argtypes = [ci, ci, ctypes.c_double, ctypes.c_double, ll, vp, vp, vp, vp, vp, vp, ci, vp,
                                 ctypes.POINTER(ctypes.c_double)]
+    lib.photons_m2l_noalloc.restype = ci
+    lib.photons_m2l_noalloc.argtypes = [ci, ci, ctypes.c_double, ctypes.c_double, ll, vp, vp, vp, vp, vp, vp, vp, ctypes.c_char_p, ci]
     lib.photons_last_error.restype = ctypes.c_char_p
     lib.photons_last_error.argtypes = [vp]
     lib.photons_destroy.restype = None
@@ -322,6 +324,37 @@ def m2l(centres, multipoles, pair_ptr, pair_src, pair_shift=None, *, p, r_s, box
     if rc != OK:
         raise PhotonsError(rc, "photons_m2l failed")
     return out, ms.value
+
+
+M2L_NOALLOC_SCRATCH_BYTES = 8 << 20      # PHOTONS_M2L_NOALLOC_SCRATCH_BYTES
+
+
+def m2l_noalloc(centres, multipoles, pair_ptr, pair_src, pair_shift=None, *, out, p, r_s, boxsize=0.0, stream=None):
+    """photons_m2l_noalloc: torch CUDA tensors only, `out` (n_cells x NC float64) supplied by the caller; enqueues on
+    `stream` (default: torch's current stream) and returns without synchronising."""
+    import torch
+
+    def ptr(x, dtype, name):
+        if x is None:
+            return None
+        if not (_is_tensor(x) and x.is_cuda and x.dtype == dtype and x.is_contiguous()):
+            raise TypeError(f"{name}: contiguous CUDA tensor of {dtype} expected")
+        return x.data_ptr()
+    n_cells = int(centres.shape[0])
+    if tuple(multipoles.shape) != (n_cells, m2l_n_coeffs(p)) or tuple(out.shape) != tuple(multipoles.shape):
+        raise ValueError("multipoles and out must be n_cells x NC(p)")
+    if stream is None:
+        stream = torch.cuda.current_stream(centres.device)
+    handle = getattr(stream, "cuda_stream", stream)
+    err = ctypes.create_string_buffer(512)
+    rc = load().photons_m2l_noalloc(centres.device.index or 0, int(p), float(r_s), float(boxsize), n_cells,
+                                    ptr(centres, torch.float64, "centres"), ptr(multipoles, torch.float64, "multipoles"),
+                                    ptr(pair_ptr, torch.int64, "pair_ptr"), ptr(pair_src, torch.int32, "pair_src"),
+                                    ptr(pair_shift, torch.int8, "pair_shift"), ptr(out, torch.float64, "out"),
+                                    ctypes.c_void_p(handle or 0), err, len(err))
+    if rc != OK:
+        raise PhotonsError(rc, err.value.decode(errors="replace"))
+    return out
 
 
 def short_range_acc(pos, mass=None, *, out=None, **params):
