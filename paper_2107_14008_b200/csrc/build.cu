@@ -432,7 +432,7 @@ __global__ void list_kernel(ListArgs a)
     const int my_cnt = a.leaf_cnt[i];
 
     int run_first = -1, run_n = 0, run_code = -1, n_chunks = 0, n_pairs = 0;
-    long long n_eval = 0;
+    long long n_src = 0;          // particles in the accepted source leaves
     // Pass 1 counts and keeps the first stash_cap entries of every leaf, and notes the state of the walk at the moment
     // the stash fills up; pass 2 (only the leaves whose list did not fit; the stashed part is copied by
     // list_copy_kernel) resumes the walk from that state and writes the rest in place.
@@ -475,14 +475,14 @@ __global__ void list_kernel(ListArgs a)
             g2 = fmaf(gap, gap, g2);
         }
         const bool accept = g2 < rc2;
-        if (accept && node < leaf0) { h = 2 * h; continue; }       // internal: down to the left child
-        if (accept) {
+        const bool internal = node < leaf0;
+        if (accept && !internal) {
             const int j = node - leaf0;
             // the three shift fields of entry_pack, without the slot count; ambiguous image -> per-pair flag (A10)
             int code = ((1 - (int)img[0]) << 16) | ((1 - (int)img[1]) << 18) | ((1 - (int)img[2]) << 20);
             if (a.periodic && 2.0f * fmaxf(hws[0], fmaxf(hws[1], hws[2])) >= amb) code = (int)entry_pack(0, 0, 0, 0, true);
             ++n_pairs;
-            n_eval += (long long)my_cnt * a.leaf_cnt[j];
+            n_src += (int)nc.w;          // the leaf's particle count rides in the box record (node_box32_kernel)
             if (run_n > 0 && j == run_first + run_n && code == run_code && run_n < max_leaves_per_chunk) {
                 ++run_n;
             } else {
@@ -493,10 +493,13 @@ __global__ void list_kernel(ListArgs a)
                 run_first = j; run_n = 1; run_code = code;
             }
         }
+        // accepted internal node: down to the left child; else on to the node after this subtree (one select: the
+        // lanes of a warp sit at different nodes, so the two ways on must not be two divergent paths)
         const unsigned up = h + 1;
-        h = up >> (__ffs(up) - 1);
-        if (h == 1) h = 0;
+        const unsigned nxt = up >> (__ffs(up) - 1);
+        h = accept && internal ? 2 * h : nxt == 1 ? 0u : nxt;
     }
+    const long long n_eval = (long long)my_cnt * n_src;
     if (run_n > 0) emit();
     if (!a.chunks) {       // whole warps arrive here
         const long long work = (long long)n_pairs * a.maxleaf;
@@ -517,7 +520,9 @@ __global__ void list_kernel(ListArgs a)
 }
 
 // fp32 boxes for the list walk: centre rounded to nearest, half-width rounded up and widened by the centre's rounding
-__global__ void node_box32_kernel(long long n_nodes, const double* __restrict__ lo, const double* __restrict__ hi, float4* __restrict__ box)
+// (.w of the centre record: the particle count of a leaf node, 0 for internal nodes - read by the list walk)
+__global__ void node_box32_kernel(long long n_nodes, long long n_leaves, const int* __restrict__ leaf_cnt,
+                                  const double* __restrict__ lo, const double* __restrict__ hi, float4* __restrict__ box)
 {
     long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (k >= n_nodes) return;
@@ -527,7 +532,8 @@ __global__ void node_box32_kernel(long long n_nodes, const double* __restrict__ 
         c[a] = (float)cd;
         h[a] = __double2float_ru(0.5 * (hi[3 * k + a] - lo[3 * k + a]) + fabs(cd - (double)c[a]));
     }
-    box[2 * k] = make_float4(c[0], c[1], c[2], 0.f);
+    const long long leaf = k - (n_leaves - 1);
+    box[2 * k] = make_float4(c[0], c[1], c[2], leaf >= 0 ? (float)leaf_cnt[leaf] : 0.f);
     box[2 * k + 1] = make_float4(h[0], h[1], h[2], 0.f);
 }
 
@@ -715,7 +721,7 @@ int build_leaves_impl(Ctx* c)
     {
         float4* box = nullptr;
         PH_WS(box, float4, WS_NODE_BOX32, 2 * n_nodes);
-        node_box32_kernel<<<blocks_for(n_nodes, tb), tb, 0, st>>>(n_nodes, c->d_node_lo, c->d_node_hi, box);
+        node_box32_kernel<<<blocks_for(n_nodes, tb), tb, 0, st>>>(n_nodes, n_leaves, c->d_leaf_cnt, c->d_node_lo, c->d_node_hi, box);
         ++c->launches;
         la.box = box;
     }
