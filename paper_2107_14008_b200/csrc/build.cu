@@ -479,7 +479,9 @@ __global__ void list_kernel(ListArgs a)
         if (accept && !internal) {
             const int j = node - leaf0;
             // the three shift fields of entry_pack, without the slot count; ambiguous image -> per-pair flag (A10)
-            int code = ((1 - (int)img[0]) << 16) | ((1 - (int)img[1]) << 18) | ((1 - (int)img[2]) << 20);
+            int code = 0x150000;                  // no image shift on any axis: almost every accepted leaf
+            if (img[0] != 0.f || img[1] != 0.f || img[2] != 0.f)
+                code = ((1 - (int)img[0]) << 16) | ((1 - (int)img[1]) << 18) | ((1 - (int)img[2]) << 20);
             if (a.periodic && 2.0f * fmaxf(hws[0], fmaxf(hws[1], hws[2])) >= amb) code = (int)entry_pack(0, 0, 0, 0, true);
             ++n_pairs;
             n_src += (int)nc.w;          // the leaf's particle count rides in the box record (node_box32_kernel)

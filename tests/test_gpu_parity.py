@@ -232,6 +232,29 @@ def test_pairs_evaluated_and_list_cover(B, c1):
     assert set(np.unique(code)) <= set(range(28))
 
 
+@pytest.mark.parametrize("n,maxleaf", [(20011, 32), (5000, 16), (100003, 64)])
+def test_pairs_evaluated_is_the_sum_over_the_list_with_ragged_leaves(B, n, maxleaf):
+    """stats.pairs_evaluated (the numerator of the bench metric) against the list it describes, exactly: the sum over
+    target leaves of (particles in the leaf) x (particles in its listed source leaves), with N chosen so that leaf
+    counts differ (ORB halves odd nodes unevenly: DESIGN.md A13).  The list walk takes a leaf's count from the box
+    record of its tree node."""
+    rng = np.random.default_rng(91)
+    pos = rng.random((n, 3)).astype(np.float32).astype(np.float64)
+    with B.Photons(n_pm=32, maxleaf=maxleaf, precision="fp64", g_mode="direct") as ph:
+        ph.set_particles(pos, np.full(n, 1.0 / n))
+        ph.build_leaves()
+        st = ph.stats()
+        _, leaf_start = ph.leaf_order()
+        ptr, first, nleaf, _ = ph.interaction_list()
+    cnt = np.diff(leaf_start)
+    assert cnt.min() < cnt.max() <= maxleaf            # ragged
+    csum = np.concatenate([[0], np.cumsum(cnt)])
+    src_per_entry = csum[first + nleaf] - csum[first]
+    tl = np.repeat(np.arange(len(cnt)), np.diff(ptr))
+    assert int((cnt[tl] * src_per_entry).sum()) == st["pairs_evaluated"]
+    assert int(nleaf.sum()) == st["n_leaf_pairs"]
+
+
 @pytest.mark.parametrize("n,maxleaf,clustered", [(32768, 32, False), (20011, 16, False), (5000, 64, False), (262144, 32, True),
                                                  (100003, 32, True), (262144, 16, True), (300007, 16, False)])
 def test_orb_tree_is_a_median_split_along_the_widest_axis(B, n, maxleaf, clustered):
