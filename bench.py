@@ -52,9 +52,9 @@ def flops_per_pair(precision: str, g_mode: str, *, poly_degree: int = POLY_DEGRE
                    table_layout: str = "paper", equal_mass: bool = False) -> float:
     """Executed flops per evaluated pair, counted in the SASS of each kernel's hot loop (profiles/r2_sass_inner_loop.md;
     ncu's op_ffma counters read 0 for the packed FFMA2 stream): FFMA/DFMA = 2, FADD/FMUL/DADD/DMUL = 1, MUFU = 1,
-    compares and selects 0.  equal_mass: the fp32 POLY / TABLE / FUSED kernels that the library takes when all masses
+    compares and selects 0.  equal_mass: the fp32 / mixed POLY / TABLE / FUSED kernels that the library takes when all masses
     are equal (photons_params.mass_path = 0) leave the multiply by G m_j out of the pair core: one FMUL per pair less."""
-    if equal_mass and precision == "fp32" and g_mode in ("poly", "table", "fused"):
+    if equal_mass and precision in ("fp32", "mixed") and g_mode in ("poly", "table", "fused"):
         return flops_per_pair(precision, g_mode, poly_degree=poly_degree, table_level=table_level, table_layout=table_layout) - 1.0
     if precision == "fp64":
         if g_mode == "direct":     # executed per pair on config 4 (ncu DFMA/DMUL/DADD counters): 52.6 + 12.7 + 7.8 + 3 MUFU;
@@ -362,8 +362,10 @@ def run_ours(args):
         peak_tf = peak_tflops(args.precision, clocks["sm_max_mhz"] or 1965.0)
         achieved_tf = pairs * fpp / (kernel_ms * 1e-3) / 1e12
         traffic, traffic_src = ncu_traffic(cfg0.name, params["maxleaf"], args.precision, args.g_mode)
-        if args.mass_path and args.precision == "fp32" and args.g_mode != "direct":
-            traffic, traffic_src = None, None      # the rows of these variants are captures of the equal-mass kernels
+        # a row stands for the kernel it was captured on: equal-mass or G m_j per pair
+        eq_kernel = not args.mass_path and args.precision in ("fp32", "mixed") and args.g_mode != "direct"
+        if traffic_src and args.precision != "fp64" and args.g_mode != "direct" and ("equal-mass kernel" in traffic_src) != eq_kernel:
+            traffic, traffic_src = None, None
         f64 = args.precision == "fp64"
         roofline = {
             "bound": "alu", "kernel": "p2p_fp64_kernel" if f64 else "p2p_fp32_kernel", "achieved": achieved_tf, "peak": peak_tf,
@@ -397,7 +399,7 @@ def run_ours(args):
             "config": {"workload": cfg0.name, "n_particles": n, "n_pm": cfg.n_pm, "maxleaf": params["maxleaf"],
                        "precision": args.precision, "g_mode": args.g_mode, "close_pair_radius_over_rcut": params["close_pair_radius"] / r_cut,
                        "n_streams": args.streams, "input_flavour": "F (fp32-grid positions)",
-                       "masses": "equal (one particle species, mass = NULL); " + ("G m_j per pair forced (mass_path 1)" if args.mass_path or args.precision != "fp32" or args.g_mode == "direct"
+                       "masses": "equal (one particle species, mass = NULL); " + ("G m_j per pair forced (mass_path 1)" if args.mass_path or args.precision == "fp64" or args.g_mode == "direct"
                                                                                    else "equal-mass kernels: G m applied once per staged run (mass_path 0)"),
                        "l2": "inputs exceed L2 (leaf-sorted particles + interaction list > 126 MB); no flush",
                        "parallelism": f"replicas x{world}" if world > 1 else "single GPU",

@@ -117,7 +117,7 @@ typedef struct {
                                  together and share their source leaves in L2), 1 = longest source list first */
     int orb_method;           /* upper levels of the ORB build: 0 = radix-select partition of every node about its median
                                  (default), 1 = one full radix sort of (node, coordinate) keys per level (round-1 path) */
-    int mass_path;            /* fp32 kernels with g_mode POLY, FUSED or TABLE: 0 = when photons_set_particles finds every mass
+    int mass_path;            /* fp32 and mixed kernels with g_mode POLY, FUSED or TABLE: 0 = when photons_set_particles finds every mass
                                  equal (one particle species, the paper's runs; Alg. 2 L177 carries a single GM) the pair core
                                  leaves G m out and applies it once per staged run (default); 1 = always G m_j per pair.
                                  Same sums up to fp32 rounding order. */

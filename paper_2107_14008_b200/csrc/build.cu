@@ -697,7 +697,7 @@ int build_leaves_impl(Ctx* c)
         double* leaf_hi = c->d_node_hi + 3 * (n_leaves - 1);
         leaf_table_kernel<<<blocks_for(n_leaves, 128), 128, 0, st>>>(n, depth, n_leaves, c->d_perm, c->d_pos, c->d_leaf_cnt, leaf_lo, leaf_hi, c->d_leaf_ctr);
         // equal masses (set_particles) and a kernel that can leave G m out of the pair core (photons_params.mass_path)
-        c->ugm = c->gm_uniform != 0.0 && c->p.mass_path == 0 && c->p.precision == PHOTONS_FP32 && c->p.g_mode != PHOTONS_G_DIRECT;
+        c->ugm = c->gm_uniform != 0.0 && c->p.mass_path == 0 && c->p.precision != PHOTONS_FP64 && c->p.g_mode != PHOTONS_G_DIRECT;
         pack_kernel<<<blocks_for(n_slots, tb), tb, 0, st>>>(n, depth, M, n_slots, c->p.G, c->p.precision, c->ugm ? 1 : 0, 1.0 / c->pscale, 1.0 / c->gmscale,
                                                             c->d_perm, c->d_pos, c->d_mass,
                                                             c->d_leaf_ctr, c->d_slot_src, c->d_p64, c->d_p32);

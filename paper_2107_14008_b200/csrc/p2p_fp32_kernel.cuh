@@ -500,6 +500,9 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
                             const float dx = image(hh ? A.y : A.x, tx[t], dc.x), dy = image(hh ? A.w : A.z, ty[t], dc.y),
                                         dz = image(hh ? B.y : B.x, tz[t], dc.z);
                             float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.r2add)));
+                            // equal-mass kernels: a padding slot sits at PAD_FAR instead of carrying zero mass, and MIXED
+                            // wraps the offset by whole box lengths here - keep it beyond the cut
+                            if (UGM && MIXED && (hh ? A.y : A.x) >= 0.5f * PAD_FAR) r2 = 3.0e30f;
                             const float2 w = weight2<GKIND, GPAR>(a, tab, dup(r2), dup(UGM ? 1.f : hh ? B.w : B.z));
                             px[t] = fmaf(w.x, dx, px[t]); py[t] = fmaf(w.x, dy, py[t]); pz[t] = fmaf(w.x, dz, pz[t]);
                         }
@@ -669,10 +672,10 @@ static int launch_p32_shape(Ctx* c, const P32Args& a, long long count, cudaStrea
     const size_t smem = p32_smem_bytes(c, T);
     void (*kern)(P32Args) = nullptr;
     const bool mixed = c->p.precision == PHOTONS_MIXED;
-    const bool ugm = c->ugm;     // equal masses: G m out of the pair core (never MIXED or DIRECT: build_leaves)
+    const bool ugm = c->ugm;     // equal masses: G m out of the pair core (never DIRECT: build_leaves)
     constexpr bool HAS_UGM = GKIND != GM_DIRECT;
-#define PH_SHAPE(TT, HH) (mixed ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR> : ugm ? p2p_fp32_kernel<TT, HH, false, GKIND, GPAR, HAS_UGM> \
-                                : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR>)
+#define PH_SHAPE(TT, HH) (mixed ? (ugm ? p2p_fp32_kernel<TT, HH, true, GKIND, GPAR, HAS_UGM> : p2p_fp32_kernel<TT, HH, true, GKIND, GPAR>) \
+                                : (ugm ? p2p_fp32_kernel<TT, HH, false, GKIND, GPAR, HAS_UGM> : p2p_fp32_kernel<TT, HH, false, GKIND, GPAR>))
     switch (M * 8 + T) {   // (MAXLEAF, targets per lane) -> (T, lane groups)
         case 16 * 8 + 1: kern = PH_SHAPE(1, 2); break;
         case 16 * 8 + 2: kern = PH_SHAPE(2, 4); break;

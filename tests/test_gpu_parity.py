@@ -433,6 +433,26 @@ def test_equal_mass_kernels(B, oracle, n, maxleaf, g_mode, tol):
     assert _err(out2, ref2) <= tol
 
 
+@pytest.mark.parametrize("n,maxleaf", [(33, 16), (40, 32), (5000, 64), (20011, 32), (20011, 16)])
+@pytest.mark.parametrize("g_mode,tol", [("poly", TOL_FP32), ("table", TOL_TABLE)])
+def test_equal_mass_kernels_mixed(B, oracle, n, maxleaf, g_mode, tol):
+    """The same for precision = mixed (offsets from the leaf origins): padding slots sit at PAD_FAR there too, and the
+    tiny cases take the per-pair minimum image, which wraps offsets by whole box lengths and must leave them far."""
+    rng = np.random.default_rng(700 + n)
+    pos = rng.random((n, 3)).astype(np.float32).astype(np.float64)
+    m0, G = 7.5 / n, 43.0
+    mass = np.full(n, m0)
+    n_pm = 16
+    r_s = 1.2 / n_pm
+    ref, _ = oracle.p2p(pos, mass, boxsize=1.0, r_s=r_s, r_cut=6 * r_s, G=G)
+    kw = dict(n_pm=n_pm, G=G, precision="mixed", g_mode=g_mode, maxleaf=maxleaf, close_pair_radius=0.02 * 6 * r_s)
+    eq, _ = B.short_range_acc(pos, mass, **kw)
+    per, _ = B.short_range_acc(pos, mass, mass_path=1, **kw)
+    assert _err(eq, ref) <= tol and _err(per, ref) <= tol
+    assert _err(eq, per) <= 0.5 * TOL_FP32
+    assert n < 1000 or not np.array_equal(eq, per)
+
+
 def test_equal_mass_kernels_softened_isolated_and_negative(B, oracle):
     rng = np.random.default_rng(91)
     n, n_pm = 6001, 16
