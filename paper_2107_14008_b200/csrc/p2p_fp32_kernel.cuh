@@ -319,7 +319,11 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
-    const int M = a.maxleaf;
+    // the leaf size is fixed by the mapping (T targets per lane, HS lane groups): a build-time constant for the MIXED
+    // kernels' walk over the source leaves of a run (trip counts and shifts known to the compiler)
+    constexpr int MC = T * 32 / HS;
+    constexpr int LOG2_MC = MC == 16 ? 4 : MC == 32 ? 5 : MC == 64 ? 6 : 7;
+    const int M = MIXED ? MC : a.maxleaf;
     const int stage_bytes = a.chunk_max * 16;
     unsigned char* ring = smem_raw + (size_t)warp * N_STAGES * stage_bytes;
     unsigned char* tail = smem_raw + (size_t)W * N_STAGES * stage_bytes;
@@ -399,9 +403,9 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
             // origin differences in fp64, rounded once (A15); computed when the copy is issued, N_STAGES runs
             // ahead of their use, so the global loads of the origins are off the critical path
             const uint2 e = make_uint2(__shfl_sync(0xffffffffu, mine.x, k & 31), __shfl_sync(0xffffffffu, mine.y, k & 31));
-            const int nleaf = (int)((e.y & 0xffffu) >> a.log2m);
+            const int nleaf = (int)((e.y & 0xffffu) >> LOG2_MC);
             if (lane < nleaf) {
-                const long long jl = (long long)(e.x >> a.log2m) + lane;
+                const long long jl = (long long)(e.x >> LOG2_MC) + lane;
                 const int sxi = (int)((e.y >> 16) & 3u) - 1, syi = (int)((e.y >> 18) & 3u) - 1, szi = (int)((e.y >> 20) & 3u) - 1;
                 cshift[st * MAX_RUN_LEAVES + lane] = make_float4((float)(((a.ctr[3 * jl] + a.Ld * sxi) - cix) * a.inv_pscale),
                                                                  (float)(((a.ctr[3 * jl + 1] + a.Ld * syi) - ciy) * a.inv_pscale),
@@ -451,7 +455,7 @@ __global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T
             float sax = 0.f, say = 0.f, saz = 0.f;
             float4 dc = make_float4(0.f, 0.f, 0.f, 0.f);
             if (MIXED) {
-                dc = cshift[st * MAX_RUN_LEAVES + (b0 >> a.log2m)];
+                dc = cshift[st * MAX_RUN_LEAVES + (b0 >> LOG2_MC)];
 #pragma unroll
                 for (int t = 0; t < T; ++t) { qx[t] = tx[t] - dc.x; qy[t] = ty[t] - dc.y; qz[t] = tz[t] - dc.z; }
             } else {
