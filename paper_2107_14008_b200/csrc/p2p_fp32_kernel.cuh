@@ -31,6 +31,13 @@
                               // instead of a select on the weight (config 4, MAXLEAF 64: 117.3 against 119.6 ms; with one target
                               // per lane it changes nothing at MAXLEAF 32 and costs 3 % at MAXLEAF 16, so it stays off there)
 #endif
+#ifndef PHOTONS_MINBLOCKS_T1
+#define PHOTONS_MINBLOCKS_T1 2   // __launch_bounds__(256, .) of the kernels with one target per lane and full-warp groups (MAXLEAF 32):
+                                 // 2 leaves the compiler the 96 registers it asks for (5 CTAs of 128 threads per SM); 3 caps it at 80
+                                 // (6 CTAs) at the price of re-computed addresses and a local-memory phase bit per list entry.
+                                 // Config 4, 2 against 3: POLY 89.8 / 90.6 ms, FUSED 96.6 / 97.9, MIXED 95.1 / 97.4, TABLE 512 99.9 / 99.8,
+                                 // TABLE 4096 104.1 / 112.9.  Half-warp groups (MAXLEAF 16) keep 3: 84.1 / 82.8 ms, MIXED 102.9 / 98.3
+#endif
 #ifndef PHOTONS_MINBLOCKS_T2
 #define PHOTONS_MINBLOCKS_T2 2   // __launch_bounds__(256, .) of the kernels with two targets per lane
 #endif
@@ -315,7 +322,7 @@ static __device__ __noinline__ double3 exact_run(const double4* __restrict__ p64
 // ---------------------------------------------------------------------------------------------------------
 
 template <int T, int HS, bool MIXED, int GKIND, int GPAR, bool UGM = false>
-__global__ void __launch_bounds__(256, T == 1 ? 3 : T == 2 ? PHOTONS_MINBLOCKS_T2 : 1) p2p_fp32_kernel(P32Args a)
+__global__ void __launch_bounds__(256, T == 1 ? (HS == 1 ? PHOTONS_MINBLOCKS_T1 : 3) : T == 2 ? PHOTONS_MINBLOCKS_T2 : 1) p2p_fp32_kernel(P32Args a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
